@@ -1,0 +1,164 @@
+/* include/haste.h -- C ABI of the HASTE hot path on one B200 (sm_100a).
+ *
+ * What it is: the group-shared fixed fan-in sparse output layer of HASTE
+ * (arxiv/paper_2606_01117) and its small dense head, forward fused with the
+ * BCE-with-logits objective, plus the full backward.  Citations are lines of the
+ * paper's text (PAPER.md:<line>):
+ *
+ *   labels are partitioned into groups of G; group g shares one support
+ *   I_g = idx[g, 0..K) of K input features, label l keeps its own K weights
+ *   W[l, 0..K):
+ *     z[i,l]  = bias[l] + sum_j W[l,j] * X[i, idx[l/G, j]]
+ *     loss    = s * sum_i sum_l ( softplus(z[i,l]) - y[i,l] z[i,l] ) PAPER.md:111 (Eq. 3), s = 1/B
+ *     dY[i,l] = s * ( sigmoid(z[i,l]) - y[i,l] )
+ *     dW[l,j] = sum_i dY[i,l] * X[i, idx[l/G, j]]
+ *     dX[i,f] = sum_l sum_{j: idx[l/G,j]=f} dY[i,l] * W[l,j]
+ *   dense head over the frequent labels: z = b + X_h W_h^T, same objective,
+ *     dW_h = dY^T X_h, dX_h = dY W_h
+ *
+ * (Paper symbols: H -> d, F -> K, number of groups K_paper -> NG = ceil(L/G).)
+ *
+ * Conventions
+ *  - Every tensor pointer is DEVICE memory owned by the caller (unless a
+ *    parameter says "host"); the library never frees or keeps it past the call.
+ *    A handle owns only its workspace (X^T copy, dX^T accumulator, loss partials,
+ *    TMA descriptors), sized from B_max at create and freed at destroy.
+ *  - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL is the
+ *    legacy default stream) and return without synchronising.  `loss` is a device
+ *    scalar.  A handle is not thread-safe: one stream at a time per handle.
+ *  - Every function returns a haste_status_t; 0 is success.  Nothing throws, aborts
+ *    or prints.  Argument errors are detected on the host before any launch.
+ *    Index CONTENTS are not checked by the hot calls; haste_validate_index does it.
+ *  - Pointers to X, W, dY, dW must be 16-byte aligned.
+ *  - idx rows may hold any values in [0,d): duplicates add, order is free
+ *    (reading R4).  HASTE_IDX_SORTED_DISTINCT is a caller's promise that
+ *    only enables faster paths.
+ *  - Targets: one CSR over GLOBAL label ids, ascending and distinct within a row;
+ *    a layer looks only at ids in [label_offset, label_offset + L).
+ *  - dY of the sparse tail lives in a library-defined layout (group-blocked:
+ *    element (i,l) at ((l/G)*B + i)*G + l%G, type `dtype`); use haste_dy_bytes,
+ *    haste_dy_unpack and haste_dy_pack to size and convert it.  dY of the head is
+ *    plain [B, L_h] row-major.
+ */
+#ifndef HASTE_H_
+#define HASTE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct haste_layer haste_layer_t; /* opaque; sparse tail */
+typedef struct haste_head haste_head_t;   /* opaque; dense head  */
+
+typedef enum {
+  HASTE_OK = 0,
+  HASTE_ERR_INVALID_ARG = -1, /* NULL required pointer, B > B_max, misaligned pointer, bad sizes */
+  HASTE_ERR_BAD_INDEX = -2,   /* haste_validate_index: value outside [0,d) or broken sorted-distinct promise */
+  HASTE_ERR_UNSUPPORTED = -3, /* shape/dtype the kernels do not cover */
+  HASTE_ERR_CUDA = -4,        /* CUDA runtime/driver error; text in haste_last_error() */
+  HASTE_ERR_NOMEM = -5
+} haste_status_t;
+
+typedef enum { HASTE_F32 = 0, HASTE_BF16 = 1 } haste_dtype_t;
+
+typedef enum {
+  HASTE_IDX_SORTED_DISTINCT = 1u, /* promise: every idx row strictly ascending */
+  HASTE_DETERMINISTIC = 2u,       /* forbid float atomics on dX (slower path) */
+  HASTE_FORCE_SIMT = 4u           /* use the generic CUDA-core kernels even where tcgen05 kernels exist */
+} haste_flags_t;
+
+typedef struct {
+  int32_t d;              /* input features (paper H)                                       */
+  int64_t L;              /* labels in THIS layer; need not be a multiple of G (R3)         */
+  int32_t G, K;           /* labels per group; fan-in per group (paper F)                   */
+  int32_t B_max;          /* largest batch any call will pass                               */
+  haste_dtype_t dtype;    /* type of X, W, dY; accumulation is always fp32                  */
+  haste_dtype_t dw_dtype; /* type of dW                                                     */
+  int64_t label_offset;   /* global id of this layer's label 0 in the targets' CSR          */
+  float loss_scale;       /* 0 -> 1/B per call (Eq. 3); otherwise used as given             */
+  uint32_t flags;         /* haste_flags_t bits                                             */
+} haste_config_t;
+
+/* ---- sparse tail ------------------------------------------- */
+
+/* Allocates the handle and its workspace on `cuda_device`.  *out is NULL on failure. */
+int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device);
+int haste_destroy(haste_layer_t* h);
+
+/* Bytes of the dY buffer for a call with batch B (NG * B * G elements of `dtype`). */
+size_t haste_dy_bytes(const haste_layer_t* h, int B);
+
+/* Checks idx [NG,K] (device): every value in [0,d) and, if the handle promised
+ * HASTE_IDX_SORTED_DISTINCT, every row strictly ascending.  Synchronises `stream`.
+ * Returns HASTE_OK or HASTE_ERR_BAD_INDEX. */
+int haste_validate_index(haste_layer_t* h, const int32_t* idx, void* stream);
+
+/* Forward + fused BCE-with-logits.  The B x L logits are not
+ * written unless logits_out is given. */
+int haste_forward_loss(haste_layer_t* h, int B,
+                       const void* X,             /* [B,d] row-major, dtype                                   */
+                       const int32_t* idx,        /* [NG,K] int32, NG = ceil(L/G); values in [0,d)            */
+                       const void* W,             /* [L,K] row-major, dtype                                   */
+                       const float* bias,         /* [L] fp32 or NULL                                         */
+                       const int32_t* tgt_rowptr, /* [B+1]                                                    */
+                       const int32_t* tgt_col,    /* [nnz] global label ids, ascending within a row           */
+                       float* loss,               /* device scalar, overwritten; NULL -> not computed         */
+                       void* dY,                  /* haste_dy_bytes(h,B), overwritten; NULL -> inference only */
+                       float* logits_out,         /* optional [B,L] row-major fp32, or NULL                   */
+                       void* stream);
+
+/* Backward from a dY in the library layout. */
+int haste_backward(haste_layer_t* h, int B,
+                   const void* X, const int32_t* idx, const void* W, const void* dY,
+                   void* dW,          /* [L,K] row-major, dw_dtype; overwritten.  NULL -> skipped */
+                   float* dbias,      /* [L] fp32, overwritten, or NULL                           */
+                   float* dX,         /* [B,d] row-major fp32.  NULL -> skipped                   */
+                   int accumulate_dX, /* 0: overwrite dX; 1: add to its contents                  */
+                   void* stream);
+
+/* dY layout helpers: library layout <-> plain [B,L] row-major fp32. */
+int haste_dy_unpack(const haste_layer_t* h, int B, const void* dY, float* out_BL, void* stream);
+int haste_dy_pack(const haste_layer_t* h, int B, const float* in_BL, void* dY, void* stream);
+
+/* ---- dense head ---------------------------------------------------- */
+
+int haste_head_create(haste_head_t** out, int32_t d, int64_t L_h, int32_t B_max, haste_dtype_t dtype,
+                      int64_t label_offset, float loss_scale, uint32_t flags, int cuda_device);
+int haste_head_destroy(haste_head_t* h);
+
+int haste_head_forward_loss(haste_head_t* h, int B,
+                            const void* X,    /* [B,d] row-major, dtype (the head's own input) */
+                            const void* Wh,   /* [L_h,d] row-major, dtype                                     */
+                            const float* bias,/* [L_h] fp32 or NULL                                           */
+                            const int32_t* tgt_rowptr, const int32_t* tgt_col,
+                            float* loss,      /* device scalar or NULL                                        */
+                            void* dY,         /* [B,L_h] row-major, dtype; NULL -> inference only             */
+                            float* logits_out,/* optional [B,L_h] fp32                                        */
+                            void* stream);
+
+int haste_head_backward(haste_head_t* h, int B, const void* X, const void* Wh, const void* dY,
+                        void* dWh,    /* [L_h,d] row-major, dtype; NULL -> skipped */
+                        float* dbias, /* [L_h] fp32 or NULL                        */
+                        float* dX,    /* [B,d] fp32; NULL -> skipped               */
+                        int accumulate_dX, void* stream);
+
+/* ---- diagnostics ---------------------------------------------------------------------- */
+
+const char* haste_status_string(int status);
+const char* haste_last_error(void); /* thread-local detail of the last failure */
+
+/* Which kernel family a handle runs: 0 = generic CUDA-core (SIMT), 1 = tcgen05/TMEM/TMA. */
+int haste_kernel_family(const haste_layer_t* h);
+int haste_head_kernel_family(const haste_head_t* h);
+
+/* Kernels the last forward / backward call on this handle launched (for bench.py's gpu_launches). */
+int haste_last_launch_count(const haste_layer_t* h);
+int haste_head_last_launch_count(const haste_head_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HASTE_H_ */

@@ -1,0 +1,454 @@
+// haste_api.cu -- the C-ABI boundary (include/haste.h): handles, argument checks,
+// workspace, kernel-family dispatch.  No arithmetic of the method lives here.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "kernels.h"
+#include "tc_kernels.h"
+
+namespace haste {
+
+static thread_local char g_err[512] = "";
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+static inline size_t esize(haste_dtype_t dt) { return dt == HASTE_F32 ? 4 : 2; }
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace haste
+
+using namespace haste;
+
+struct haste_layer {
+  haste_config_t cfg;
+  int device;
+  int family;       // 0 SIMT, 1 tcgen05
+  int64_t NG;
+  int Bpad;         // row pitch of Xt / dXt
+  void* Xt;         // [d][Bpad] dtype
+  float* dXt;       // [d][Bpad] fp32
+  double* loss_acc; // device scalar
+  float* partials;  // [n_partials] per-CTA loss partials (tcgen05 family)
+  int n_partials;
+  int* flag;        // validate_index result
+  TcTailState* tc;  // tcgen05 family state (tensor maps, counters) or NULL
+  int last_launches;
+};
+
+struct haste_head {
+  int32_t d;
+  int64_t L;
+  int32_t B_max;
+  haste_dtype_t dtype;
+  int64_t label_offset;
+  float loss_scale;
+  uint32_t flags;
+  int device;
+  int family;
+  double* loss_acc;
+  float* partials;
+  int n_partials;
+  TcHeadState* tc;
+  int last_launches;
+};
+
+extern "C" {
+
+const char* haste_status_string(int status) {
+  switch (status) {
+    case HASTE_OK: return "HASTE_OK";
+    case HASTE_ERR_INVALID_ARG: return "HASTE_ERR_INVALID_ARG";
+    case HASTE_ERR_BAD_INDEX: return "HASTE_ERR_BAD_INDEX";
+    case HASTE_ERR_UNSUPPORTED: return "HASTE_ERR_UNSUPPORTED";
+    case HASTE_ERR_CUDA: return "HASTE_ERR_CUDA";
+    case HASTE_ERR_NOMEM: return "HASTE_ERR_NOMEM";
+    default: return "HASTE_ERR_UNKNOWN";
+  }
+}
+
+const char* haste_last_error(void) { return g_err; }
+
+int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device) {
+  if (!out) { set_error("haste_create: out is NULL"); return HASTE_ERR_INVALID_ARG; }
+  *out = nullptr;
+  if (!cfg) { set_error("haste_create: cfg is NULL"); return HASTE_ERR_INVALID_ARG; }
+  if (cfg->d <= 0 || cfg->L < 0 || cfg->G <= 0 || cfg->K <= 0 || cfg->B_max <= 0) {
+    set_error("haste_create: d, G, K, B_max must be positive and L >= 0");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if ((cfg->dtype != HASTE_F32 && cfg->dtype != HASTE_BF16) || (cfg->dw_dtype != HASTE_F32 && cfg->dw_dtype != HASTE_BF16)) {
+    set_error("haste_create: unknown dtype");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (cfg->flags & HASTE_DETERMINISTIC) {
+    set_error("haste_create: HASTE_DETERMINISTIC (atomic-free dX) is not implemented yet");
+    return HASTE_ERR_UNSUPPORTED;
+  }
+  if (cfg->G > 1024 || cfg->K > 4096) {
+    set_error("haste_create: G <= 1024 and K <= 4096 are supported");
+    return HASTE_ERR_UNSUPPORTED;
+  }
+  const int64_t NG = (cfg->L + cfg->G - 1) / cfg->G;
+  if (NG > 0x7fffffffLL) { set_error("haste_create: too many groups"); return HASTE_ERR_UNSUPPORTED; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
+    cudaGetLastError();
+    set_error("haste_create: CUDA device %d not available (no CPU fallback exists)", cuda_device);
+    return HASTE_ERR_CUDA;
+  }
+  DeviceGuard guard(cuda_device);
+  if (!guard.ok) { set_error("haste_create: cudaSetDevice failed"); return HASTE_ERR_CUDA; }
+  haste_layer* h = new (std::nothrow) haste_layer();
+  if (!h) return HASTE_ERR_NOMEM;
+  memset(h, 0, sizeof(*h));
+  h->cfg = *cfg;
+  h->device = cuda_device;
+  h->NG = NG;
+  h->Bpad = round_up(cfg->B_max, 128);
+  h->n_partials = 1024;
+  const size_t xt_bytes = (size_t)cfg->d * h->Bpad * esize(cfg->dtype);
+  const size_t dxt_bytes = (size_t)cfg->d * h->Bpad * 4;
+  cudaError_t e = cudaMalloc(&h->Xt, xt_bytes);
+  if (e == cudaSuccess) e = cudaMalloc(&h->dXt, dxt_bytes);
+  if (e == cudaSuccess) e = cudaMalloc(&h->loss_acc, sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&h->partials, h->n_partials * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&h->flag, sizeof(int));
+  if (e == cudaSuccess) e = cudaMemset(h->Xt, 0, xt_bytes);
+  if (e == cudaSuccess) e = cudaMemset(h->partials, 0, h->n_partials * sizeof(float));
+  if (e != cudaSuccess) {
+    set_error("haste_create: workspace allocation failed: %s", cudaGetErrorString(e));
+    haste_destroy(h);
+    return e == cudaErrorMemoryAllocation ? HASTE_ERR_NOMEM : HASTE_ERR_CUDA;
+  }
+  h->family = 0;
+  if (!(cfg->flags & HASTE_FORCE_SIMT) && tc_tail_supported(*cfg, cuda_device)) {
+    int rc = tc_tail_create(&h->tc, *cfg, h->Bpad, cuda_device);
+    if (rc != HASTE_OK) { haste_destroy(h); return rc; }
+    h->family = 1;
+  }
+  *out = h;
+  return HASTE_OK;
+}
+
+int haste_destroy(haste_layer_t* h) {
+  if (!h) return HASTE_OK;
+  DeviceGuard guard(h->device);
+  if (h->tc) tc_tail_destroy(h->tc);
+  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag);
+  delete h;
+  return HASTE_OK;
+}
+
+size_t haste_dy_bytes(const haste_layer_t* h, int B) {
+  if (!h || B < 0) return 0;
+  return (size_t)h->NG * (size_t)B * (size_t)h->cfg.G * esize(h->cfg.dtype);
+}
+
+int haste_kernel_family(const haste_layer_t* h) { return h ? h->family : -1; }
+int haste_last_launch_count(const haste_layer_t* h) { return h ? h->last_launches : 0; }
+
+int haste_validate_index(haste_layer_t* h, const int32_t* idx, void* stream) {
+  if (!h || !idx) { set_error("haste_validate_index: NULL argument"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  HASTE_CUDA_TRY(cudaMemsetAsync(h->flag, 0, sizeof(int), st));
+  int rc = launch_validate_index(idx, h->NG, h->cfg.K, h->cfg.d, (h->cfg.flags & HASTE_IDX_SORTED_DISTINCT) ? 1 : 0,
+                                 h->flag, st);
+  if (rc != HASTE_OK) return rc;
+  int flag = 0;
+  HASTE_CUDA_TRY(cudaMemcpyAsync(&flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+  HASTE_CUDA_TRY(cudaStreamSynchronize(st));
+  if (flag & 1) { set_error("haste_validate_index: value outside [0,d)"); return HASTE_ERR_BAD_INDEX; }
+  if (flag & 2) { set_error("haste_validate_index: a row is not strictly ascending"); return HASTE_ERR_BAD_INDEX; }
+  return HASTE_OK;
+}
+
+static int check_call(const haste_layer_t* h, int B, const char* fn) {
+  if (!h) { set_error("%s: handle is NULL", fn); return HASTE_ERR_INVALID_ARG; }
+  if (B < 0 || B > h->cfg.B_max) { set_error("%s: B=%d outside [0, B_max=%d]", fn, B, h->cfg.B_max); return HASTE_ERR_INVALID_ARG; }
+  return HASTE_OK;
+}
+
+static TailShape make_shape(const haste_layer_t* h, int B) {
+  TailShape sh;
+  sh.d = h->cfg.d; sh.G = h->cfg.G; sh.K = h->cfg.K; sh.B = B; sh.Bpad = h->Bpad;
+  sh.L = h->cfg.L; sh.NG = h->NG; sh.label_offset = h->cfg.label_offset;
+  sh.s = h->cfg.loss_scale != 0.f ? h->cfg.loss_scale : (B > 0 ? 1.0f / (float)B : 0.f);
+  return sh;
+}
+
+int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias,
+                       const int32_t* tgt_rowptr, const int32_t* tgt_col, float* loss, void* dY, float* logits_out,
+                       void* stream) {
+  int rc = check_call(h, B, "haste_forward_loss");
+  if (rc) return rc;
+  if (!X || !idx || !W) { set_error("haste_forward_loss: X, idx and W are required"); return HASTE_ERR_INVALID_ARG; }
+  if ((tgt_rowptr == nullptr) != (tgt_col == nullptr)) {
+    set_error("haste_forward_loss: tgt_rowptr and tgt_col must both be given or both be NULL");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(dY) || !aligned16(idx)) {
+    set_error("haste_forward_loss: X, W, idx and dY must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const TailShape sh = make_shape(h, B);
+  h->last_launches = 0;
+  if (B == 0 || h->NG == 0) {
+    if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(loss, 0, sizeof(float), st));
+    return HASTE_OK;
+  }
+  rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+  if (rc) return rc;
+  h->last_launches++;
+  if (h->family == 1) {
+    int n = 0;
+    rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY,
+                         logits_out, st, &n);
+    if (rc) return rc;
+    h->last_launches += n;
+    if (loss) {
+      rc = launch_finalize_loss(nullptr, h->partials, tc_tail_num_partials(h->tc), sh.s, loss, st);
+      if (rc) return rc;
+      h->last_launches++;
+    }
+    return HASTE_OK;
+  }
+  if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(h->loss_acc, 0, sizeof(double), st));
+  rc = launch_simt_forward(h->cfg.dtype, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->loss_acc : nullptr, dY,
+                           logits_out, st);
+  if (rc) return rc;
+  h->last_launches++;
+  if (loss) {
+    rc = launch_finalize_loss(h->loss_acc, nullptr, 0, sh.s, loss, st);
+    if (rc) return rc;
+    h->last_launches++;
+  }
+  return HASTE_OK;
+}
+
+int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const void* dY, void* dW,
+                   float* dbias, float* dX, int accumulate_dX, void* stream) {
+  int rc = check_call(h, B, "haste_backward");
+  if (rc) return rc;
+  if (!X || !idx || !W || !dY) { set_error("haste_backward: X, idx, W and dY are required"); return HASTE_ERR_INVALID_ARG; }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(dY) || !aligned16(dW) || !aligned16(idx)) {
+    set_error("haste_backward: X, W, idx, dY and dW must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const TailShape sh = make_shape(h, B);
+  h->last_launches = 0;
+  if (B == 0 || h->NG == 0) {
+    if (dW && h->cfg.L > 0)
+      HASTE_CUDA_TRY(cudaMemsetAsync(dW, 0, (size_t)h->cfg.L * h->cfg.K * esize(h->cfg.dw_dtype), st));
+    if (dbias && h->cfg.L > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dbias, 0, (size_t)h->cfg.L * 4, st));
+    if (dX && !accumulate_dX && B > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dX, 0, (size_t)B * sh.d * 4, st));
+    return HASTE_OK;
+  }
+  // The gather operand X^T is rebuilt here: backward must not depend on which forward ran last.
+  rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+  if (rc) return rc;
+  h->last_launches++;
+  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+  if (h->family == 1) {
+    int n = 0;
+    rc = tc_tail_backward(h->tc, sh, h->Xt, idx, W, dY, dW, dbias, dX ? h->dXt : nullptr, st, &n);
+    if (rc) return rc;
+    h->last_launches += n;
+  } else {
+    if (dW || dbias) {
+      rc = launch_simt_dw(h->cfg.dtype, h->cfg.dw_dtype, sh, h->Xt, idx, dY, dW, dbias, st);
+      if (rc) return rc;
+      h->last_launches++;
+    }
+    if (dX) {
+      rc = launch_simt_dx(h->cfg.dtype, sh, idx, W, dY, h->dXt, st);
+      if (rc) return rc;
+      h->last_launches++;
+    }
+  }
+  if (dX) {
+    rc = launch_untranspose_f32(h->dXt, dX, B, sh.d, h->Bpad, accumulate_dX, st);
+    if (rc) return rc;
+    h->last_launches++;
+  }
+  return HASTE_OK;
+}
+
+int haste_dy_unpack(const haste_layer_t* h, int B, const void* dY, float* out_BL, void* stream) {
+  int rc = check_call(h, B, "haste_dy_unpack");
+  if (rc) return rc;
+  if (!dY || !out_BL) { set_error("haste_dy_unpack: NULL argument"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  return launch_dy_unpack(h->cfg.dtype, dY, out_BL, B, h->cfg.L, h->cfg.G, (cudaStream_t)stream);
+}
+
+int haste_dy_pack(const haste_layer_t* h, int B, const float* in_BL, void* dY, void* stream) {
+  int rc = check_call(h, B, "haste_dy_pack");
+  if (rc) return rc;
+  if (!dY || !in_BL) { set_error("haste_dy_pack: NULL argument"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  return launch_dy_pack(h->cfg.dtype, in_BL, dY, B, h->cfg.L, h->cfg.G, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------
+// dense head
+// ---------------------------------------------------------------------------------
+int haste_head_create(haste_head_t** out, int32_t d, int64_t L_h, int32_t B_max, haste_dtype_t dtype,
+                      int64_t label_offset, float loss_scale, uint32_t flags, int cuda_device) {
+  if (!out) { set_error("haste_head_create: out is NULL"); return HASTE_ERR_INVALID_ARG; }
+  *out = nullptr;
+  if (d <= 0 || L_h < 0 || B_max <= 0 || L_h > 0x7fffffffLL || (dtype != HASTE_F32 && dtype != HASTE_BF16)) {
+    set_error("haste_head_create: bad sizes or dtype");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
+    cudaGetLastError();
+    set_error("haste_head_create: CUDA device %d not available (no CPU fallback exists)", cuda_device);
+    return HASTE_ERR_CUDA;
+  }
+  DeviceGuard guard(cuda_device);
+  haste_head* h = new (std::nothrow) haste_head();
+  if (!h) return HASTE_ERR_NOMEM;
+  memset(h, 0, sizeof(*h));
+  h->d = d; h->L = L_h; h->B_max = B_max; h->dtype = dtype; h->label_offset = label_offset;
+  h->loss_scale = loss_scale; h->flags = flags; h->device = cuda_device;
+  h->n_partials = 1024;
+  cudaError_t e = cudaMalloc(&h->loss_acc, sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&h->partials, h->n_partials * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemset(h->partials, 0, h->n_partials * sizeof(float));
+  if (e != cudaSuccess) {
+    set_error("haste_head_create: allocation failed: %s", cudaGetErrorString(e));
+    haste_head_destroy(h);
+    return HASTE_ERR_CUDA;
+  }
+  h->family = 0;
+  if (!(flags & HASTE_FORCE_SIMT) && tc_head_supported(d, L_h, B_max, dtype, cuda_device)) {
+    int rc = tc_head_create(&h->tc, d, L_h, B_max, cuda_device);
+    if (rc != HASTE_OK) { haste_head_destroy(h); return rc; }
+    h->family = 1;
+  }
+  *out = h;
+  return HASTE_OK;
+}
+
+int haste_head_destroy(haste_head_t* h) {
+  if (!h) return HASTE_OK;
+  DeviceGuard guard(h->device);
+  if (h->tc) tc_head_destroy(h->tc);
+  cudaFree(h->loss_acc); cudaFree(h->partials);
+  delete h;
+  return HASTE_OK;
+}
+
+int haste_head_kernel_family(const haste_head_t* h) { return h ? h->family : -1; }
+int haste_head_last_launch_count(const haste_head_t* h) { return h ? h->last_launches : 0; }
+
+static HeadShape make_head_shape(const haste_head_t* h, int B) {
+  HeadShape sh;
+  sh.d = h->d; sh.B = B; sh.L = h->L; sh.label_offset = h->label_offset;
+  sh.s = h->loss_scale != 0.f ? h->loss_scale : (B > 0 ? 1.0f / (float)B : 0.f);
+  return sh;
+}
+
+int haste_head_forward_loss(haste_head_t* h, int B, const void* X, const void* Wh, const float* bias,
+                            const int32_t* tgt_rowptr, const int32_t* tgt_col, float* loss, void* dY,
+                            float* logits_out, void* stream) {
+  if (!h) { set_error("haste_head_forward_loss: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
+  if (B < 0 || B > h->B_max) { set_error("haste_head_forward_loss: B=%d outside [0, B_max=%d]", B, h->B_max); return HASTE_ERR_INVALID_ARG; }
+  if (!X || !Wh) { set_error("haste_head_forward_loss: X and Wh are required"); return HASTE_ERR_INVALID_ARG; }
+  if ((tgt_rowptr == nullptr) != (tgt_col == nullptr)) {
+    set_error("haste_head_forward_loss: tgt_rowptr and tgt_col must both be given or both be NULL");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (!aligned16(X) || !aligned16(Wh) || !aligned16(dY)) {
+    set_error("haste_head_forward_loss: X, Wh and dY must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const HeadShape sh = make_head_shape(h, B);
+  h->last_launches = 0;
+  if (B == 0 || h->L == 0) {
+    if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(loss, 0, sizeof(float), st));
+    return HASTE_OK;
+  }
+  int rc;
+  if (h->family == 1) {
+    int n = 0;
+    rc = tc_head_forward(h->tc, sh, X, Wh, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY, logits_out, st, &n);
+    if (rc) return rc;
+    h->last_launches += n;
+    if (loss) {
+      rc = launch_finalize_loss(nullptr, h->partials, tc_head_num_partials(h->tc), sh.s, loss, st);
+      if (rc) return rc;
+      h->last_launches++;
+    }
+    return HASTE_OK;
+  }
+  if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(h->loss_acc, 0, sizeof(double), st));
+  rc = launch_simt_head_forward(h->dtype, sh, X, Wh, bias, tgt_rowptr, tgt_col, loss ? h->loss_acc : nullptr, dY,
+                                logits_out, st);
+  if (rc) return rc;
+  h->last_launches++;
+  if (loss) {
+    rc = launch_finalize_loss(h->loss_acc, nullptr, 0, sh.s, loss, st);
+    if (rc) return rc;
+    h->last_launches++;
+  }
+  return HASTE_OK;
+}
+
+int haste_head_backward(haste_head_t* h, int B, const void* X, const void* Wh, const void* dY, void* dWh, float* dbias,
+                        float* dX, int accumulate_dX, void* stream) {
+  if (!h) { set_error("haste_head_backward: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
+  if (B < 0 || B > h->B_max) { set_error("haste_head_backward: B=%d outside [0, B_max=%d]", B, h->B_max); return HASTE_ERR_INVALID_ARG; }
+  if (!X || !Wh || !dY) { set_error("haste_head_backward: X, Wh and dY are required"); return HASTE_ERR_INVALID_ARG; }
+  if (!aligned16(X) || !aligned16(Wh) || !aligned16(dY) || !aligned16(dWh)) {
+    set_error("haste_head_backward: X, Wh, dY and dWh must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const HeadShape sh = make_head_shape(h, B);
+  h->last_launches = 0;
+  if (B == 0 || h->L == 0) {
+    if (dWh && h->L > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dWh, 0, (size_t)h->L * h->d * esize(h->dtype), st));
+    if (dbias && h->L > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dbias, 0, (size_t)h->L * 4, st));
+    if (dX && !accumulate_dX && B > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dX, 0, (size_t)B * h->d * 4, st));
+    return HASTE_OK;
+  }
+  if (h->family == 1) {
+    int n = 0;
+    int rc = tc_head_backward(h->tc, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, st, &n);
+    if (rc) return rc;
+    h->last_launches += n;
+    return HASTE_OK;
+  }
+  int rc = launch_simt_head_backward(h->dtype, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, st);
+  if (rc) return rc;
+  h->last_launches += (dWh ? 1 : 0) + (dX ? 1 : 0) + (dbias ? 1 : 0);
+  return HASTE_OK;
+}
+
+}  // extern "C"

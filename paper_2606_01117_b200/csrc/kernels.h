@@ -1,0 +1,40 @@
+// kernels.h -- launcher declarations shared by the C-ABI layer (haste_api.cu) and the
+// kernel translation units.  Every launcher enqueues on `st` and returns a haste_status_t.
+#pragma once
+#include "common.cuh"
+
+namespace haste {
+
+// ---- prep / utility kernels (util_kernels.cu) ----
+// Xt[f][b] = X[b][f] for b < B, 0 for B <= b < Bzero (Bzero <= Bpad, the row pitch).
+int launch_transpose_pad(haste_dtype_t dt, const void* X, void* Xt, int B, int d, int Bpad, int Bzero, cudaStream_t st);
+// dX[b][f] (=|+=) dXt[f][b]
+int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st);
+int launch_finalize_loss(const double* acc, const float* partials, int n_partials, float scale, float* loss, cudaStream_t st);
+int launch_dy_unpack(haste_dtype_t dt, const void* dY, float* out_BL, int B, int64_t L, int G, cudaStream_t st);
+int launch_dy_pack(haste_dtype_t dt, const float* in_BL, void* dY, int B, int64_t L, int G, cudaStream_t st);
+int launch_validate_index(const int32_t* idx, int64_t NG, int K, int d, int check_sorted, int* flag, cudaStream_t st);
+
+// ---- generic CUDA-core family (simt_kernels.cu): any G, K, d; fp32 or bf16 storage ----
+int launch_simt_forward(haste_dtype_t dt, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
+                        const float* bias, const int32_t* rowptr, const int32_t* col, double* loss_acc, void* dY,
+                        float* logits_out, cudaStream_t st);
+int launch_simt_dw(haste_dtype_t dt, haste_dtype_t dw_dt, const TailShape& sh, const void* Xt, const int32_t* idx,
+                   const void* dY, void* dW, float* dbias, cudaStream_t st);
+int launch_simt_dx(haste_dtype_t dt, const TailShape& sh, const int32_t* idx, const void* W, const void* dY,
+                   float* dXt, cudaStream_t st);
+
+// Dense head, CUDA-core family.
+struct HeadShape {
+  int d, B;
+  int64_t L;
+  int64_t label_offset;
+  float s;
+};
+int launch_simt_head_forward(haste_dtype_t dt, const HeadShape& sh, const void* X, const void* Wh, const float* bias,
+                             const int32_t* rowptr, const int32_t* col, double* loss_acc, void* dY, float* logits_out,
+                             cudaStream_t st);
+int launch_simt_head_backward(haste_dtype_t dt, const HeadShape& sh, const void* X, const void* Wh, const void* dY,
+                              void* dWh, float* dbias, float* dX, int accumulate_dX, cudaStream_t st);
+
+}  // namespace haste

@@ -1,0 +1,34 @@
+// tc_kernels.h -- interface of the tcgen05 / TMEM / TMA kernel family (sm_100a) to the
+// C-ABI layer.  bf16 storage, fp32 accumulate.  See tc_tail.cu / tc_head.cu.
+#pragma once
+#include "common.cuh"
+#include "kernels.h"
+
+namespace haste {
+
+struct TcTailState;
+struct TcHeadState;
+
+// Shapes the tcgen05 sparse-tail kernels cover (everything else runs the SIMT family).
+bool tc_tail_supported(const haste_config_t& cfg, int device);
+int tc_tail_create(TcTailState** out, const haste_config_t& cfg, int Bpad, int device);
+void tc_tail_destroy(TcTailState* s);
+int tc_tail_num_partials(const TcTailState* s);
+// loss_partials: per-CTA unscaled loss partials [tc_tail_num_partials] or NULL.
+int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
+                    const float* bias, const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY,
+                    float* logits_out, cudaStream_t st, int* n_launches);
+int tc_tail_backward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
+                     const void* dY, void* dW, float* dbias, float* dXt, cudaStream_t st, int* n_launches);
+
+bool tc_head_supported(int d, int64_t L_h, int B_max, haste_dtype_t dtype, int device);
+int tc_head_create(TcHeadState** out, int d, int64_t L_h, int B_max, int device);
+void tc_head_destroy(TcHeadState* s);
+int tc_head_num_partials(const TcHeadState* s);
+int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const float* bias,
+                    const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
+                    cudaStream_t st, int* n_launches);
+int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const void* dY, void* dWh,
+                     float* dbias, float* dX, int accumulate_dX, cudaStream_t st, int* n_launches);
+
+}  // namespace haste

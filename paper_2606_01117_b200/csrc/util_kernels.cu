@@ -1,0 +1,158 @@
+// util_kernels.cu -- prep and utility kernels of the HASTE path:
+//   X -> X^T (zero-padded batch columns) so that "gather K features" is a gather of K
+//   contiguous rows (gather-once); dX^T -> dX; loss finalisation; dY
+//   layout pack/unpack; index validation.
+#include "kernels.h"
+
+namespace haste {
+
+// ---------------------------------------------------------------------------------
+// Xt[f][b] = X[b][f]; columns B..Bzero-1 are written as zeros.  32x32 smem tile.
+// ---------------------------------------------------------------------------------
+template <typename T>
+__global__ void transpose_pad_kernel(const T* __restrict__ X, T* __restrict__ Xt, int B, int d, int Bpad, int Bzero) {
+  __shared__ T tile[32][33];
+  const int f0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+  const int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+#pragma unroll
+  for (int r = ty; r < 32; r += 8) {
+    const int b = b0 + r, f = f0 + tx;
+    T v = from_f32<T>(0.f);
+    if (b < B && f < d) v = X[(int64_t)b * d + f];
+    tile[r][tx] = v;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int r = ty; r < 32; r += 8) {
+    const int f = f0 + r, b = b0 + tx;
+    if (f < d && b < Bzero) Xt[(int64_t)f * Bpad + b] = tile[tx][r];
+  }
+}
+
+int launch_transpose_pad(haste_dtype_t dt, const void* X, void* Xt, int B, int d, int Bpad, int Bzero, cudaStream_t st) {
+  dim3 grid(ceil_div(d, 32), ceil_div(Bzero, 32)), block(32, 8);
+  if (dt == HASTE_F32)
+    transpose_pad_kernel<float><<<grid, block, 0, st>>>((const float*)X, (float*)Xt, B, d, Bpad, Bzero);
+  else
+    transpose_pad_kernel<bf16><<<grid, block, 0, st>>>((const bf16*)X, (bf16*)Xt, B, d, Bpad, Bzero);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+// dX[b][f] (=|+=) dXt[f][b]
+__global__ void untranspose_f32_kernel(const float* __restrict__ dXt, float* __restrict__ dX, int B, int d, int Bpad,
+                                       int accumulate) {
+  __shared__ float tile[32][33];
+  const int b0 = blockIdx.x * 32, f0 = blockIdx.y * 32;
+  const int tx = threadIdx.x, ty = threadIdx.y;
+#pragma unroll
+  for (int r = ty; r < 32; r += 8) {
+    const int f = f0 + r, b = b0 + tx;
+    tile[r][tx] = (f < d && b < B) ? dXt[(int64_t)f * Bpad + b] : 0.f;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int r = ty; r < 32; r += 8) {
+    const int b = b0 + r, f = f0 + tx;
+    if (b < B && f < d) {
+      float v = tile[tx][r];
+      float* p = dX + (int64_t)b * d + f;
+      if (accumulate) v += *p;
+      *p = v;
+    }
+  }
+}
+
+int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st) {
+  dim3 grid(ceil_div(B, 32), ceil_div(d, 32)), block(32, 8);
+  untranspose_f32_kernel<<<grid, block, 0, st>>>(dXt, dX, B, d, Bpad, accumulate);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+// loss = scale * (acc + sum(partials[0..n)))  -- one thread, fixed order: deterministic.
+__global__ void finalize_loss_kernel(const double* acc, const float* partials, int n, float scale, float* loss) {
+  __shared__ double red[256];
+  double v = 0.0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) v += (double)partials[i];
+  red[threadIdx.x] = v;
+  __syncthreads();
+  for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+    if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *loss = (float)((double)scale * ((acc ? *acc : 0.0) + red[0]));
+}
+
+int launch_finalize_loss(const double* acc, const float* partials, int n_partials, float scale, float* loss,
+                         cudaStream_t st) {
+  finalize_loss_kernel<<<1, 256, 0, st>>>(acc, partials, n_partials, scale, loss);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+// dY library layout: element (i,l) at ((l/G)*B + i)*G + l%G.
+template <typename T>
+__global__ void dy_unpack_kernel(const T* __restrict__ dY, float* __restrict__ out, int B, int64_t L, int G) {
+  const int64_t n = (int64_t)B * L;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = e / L, l = e % L;
+    out[e] = to_f32(dY[((l / G) * B + i) * G + (l % G)]);
+  }
+}
+template <typename T>
+__global__ void dy_pack_kernel(const float* __restrict__ in, T* __restrict__ dY, int B, int64_t L, int G, int64_t NG) {
+  const int64_t n = NG * B * G;  // padding labels (>= L) of the last group are written as zero
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t g = e / ((int64_t)B * G), r = e % ((int64_t)B * G);
+    const int64_t i = r / G, l = g * G + r % G;
+    dY[e] = from_f32<T>(l < L ? in[i * L + l] : 0.f);
+  }
+}
+
+int launch_dy_unpack(haste_dtype_t dt, const void* dY, float* out_BL, int B, int64_t L, int G, cudaStream_t st) {
+  const int64_t n = (int64_t)B * L;
+  const int blocks = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+  if (n == 0) return HASTE_OK;
+  if (dt == HASTE_F32)
+    dy_unpack_kernel<float><<<blocks, 256, 0, st>>>((const float*)dY, out_BL, B, L, G);
+  else
+    dy_unpack_kernel<bf16><<<blocks, 256, 0, st>>>((const bf16*)dY, out_BL, B, L, G);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+int launch_dy_pack(haste_dtype_t dt, const float* in_BL, void* dY, int B, int64_t L, int G, cudaStream_t st) {
+  const int64_t NG = (L + G - 1) / G, n = NG * B * G;
+  if (n == 0) return HASTE_OK;
+  const int blocks = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+  if (dt == HASTE_F32)
+    dy_pack_kernel<float><<<blocks, 256, 0, st>>>(in_BL, (float*)dY, B, L, G, NG);
+  else
+    dy_pack_kernel<bf16><<<blocks, 256, 0, st>>>(in_BL, (bf16*)dY, B, L, G, NG);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+// flag |= 1 if any value is outside [0,d); flag |= 2 if check_sorted and a row is not strictly ascending.
+__global__ void validate_index_kernel(const int32_t* __restrict__ idx, int64_t n, int K, int d, int check_sorted,
+                                      int* flag) {
+  int bad = 0;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    const int v = idx[e];
+    if (v < 0 || v >= d) bad |= 1;
+    if (check_sorted && (e % K) != 0 && idx[e - 1] >= v) bad |= 2;
+  }
+  if (bad) atomicOr(flag, bad);
+}
+
+int launch_validate_index(const int32_t* idx, int64_t NG, int K, int d, int check_sorted, int* flag, cudaStream_t st) {
+  const int64_t n = NG * K;
+  if (n == 0) return HASTE_OK;
+  const int blocks = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+  validate_index_kernel<<<blocks, 256, 0, st>>>(idx, n, K, d, check_sorted, flag);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+}  // namespace haste
