@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- one-line JSON benchmark of the HASTE hot path on B200.
+
+A step = one pass of the whole hot path over one synthetic batch of BASELINE.json config 3
+(670K labels: B=512, d=768, tail 653 707 labels G=64 K=128, dense head 16 384 labels, bf16):
+  haste_forward_loss + haste_backward (sparse tail) + haste_head_forward_loss + haste_head_backward.
+`value` = algorithmic TFLOP/s of the step (2*B*L_t*K per tail pass x3 + 2*B*L_h*d per head pass x3),
+inputs resident in HBM; `e2e` = the same with the step's inputs (X, X_head, CSR targets) copied from
+pinned host memory and the step's results (losses, dX, dX_head) copied back, every step.
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+Multi-GPU: the path does not shard ("replicas only"): N ranks run N independent replicas.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOAD = "670k"
+
+
+def _flops(cfg):
+    tail = 2.0 * cfg.B * cfg.L_t * cfg.K
+    head = 2.0 * cfg.B * cfg.L_h * cfg.d
+    return tail, head
+
+
+def _alg_bytes(cfg, dw_bytes=2):
+    """Algorithmic HBM bytes per launch of each tail kernel."""
+    W = cfg.L_t * cfg.K * 2
+    idx = cfg.NG * cfg.K * 4
+    dY = cfg.NG * cfg.G * cfg.B * 2
+    X = cfg.B * cfg.d * 2
+    dX = cfg.B * cfg.d * 4
+    return {
+        "forward": W + idx + X + dY,
+        "dW": dY + idx + X + cfg.L_t * cfg.K * dw_bytes + cfg.L_t * 4,
+        "dX": dY + W + idx + dX,
+    }
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        m = json.load(open(p))
+        return dict(hbm=float(m["hbm_gbs"]), bf16=float(m["bf16_tflops"]), bf16_sustained=float(m.get("bf16_tflops_sustained", m["bf16_tflops"])), source="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.f = None
+
+    def start(self):
+        try:
+            self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if not self.proc:
+            return out
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                   "samples": len(sm), "reasons": sorted(reasons)}
+        return out
+
+
+def _sample_inputs(cfg, n_groups):
+    """A bounded sample of the workload for the CPU oracle: the first n_groups groups of the tail
+    (same B, d, G, K, same generators) and the first 64*n_groups/4 head labels."""
+    from paper_2606_01117_b200 import synth
+    import dataclasses
+    Lt = n_groups * cfg.G
+    Lh = max(16, min(cfg.L_h, n_groups * 4))
+    small = dataclasses.replace(cfg, L=Lt + Lh, L_h=Lh)
+    return small, synth.make_inputs(small, with_head=True)
+
+
+def _oracle_step(oracle, small, inp):
+    r = oracle.tail_forward(inp.X, inp.idx, inp.W, None, inp.rowptr, inp.col, small.G, label_offset=small.L_h, want_z=False)
+    oracle.tail_backward(inp.X, inp.idx, inp.W, r["dY"], small.G)
+    h = oracle.head_forward(inp.X_head, inp.W_head, None, inp.rowptr, inp.col, want_z=False)
+    oracle.head_backward(inp.X_head, inp.W_head, h["dY"])
+
+
+def cpu_baseline(cfg, target_s=12.0):
+    """The oracle as it stands, one thread, on a bounded sample sized to about target_s seconds."""
+    import oracle
+    small, inp = _sample_inputs(cfg, 4)
+    t0 = time.perf_counter()
+    _oracle_step(oracle, small, inp)
+    t1 = time.perf_counter() - t0
+    ng = int(max(4, min(cfg.NG, 4 * target_s / max(t1, 1e-3))))
+    small, inp = _sample_inputs(cfg, ng)
+    t0 = time.perf_counter()
+    _oracle_step(oracle, small, inp)
+    dt = time.perf_counter() - t0
+    tail, head = _flops(small)
+    fl = 3 * (tail + head)
+    return {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": 1, "kind": "oracle",
+            "sample": "first %d of %d tail groups (%d labels) + %d head labels of config 3, B=%d, one fwd+bwd pass, %.1f s"
+                      % (ng, cfg.NG, small.L_t, small.L_h, cfg.B, dt)}
+
+
+def run_reference(args, cfg):
+    """--impl reference: the fp64 oracle, one thread, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    ng = 8
+    small, inp = _sample_inputs(cfg, ng)
+    for _ in range(args.warmup):
+        _oracle_step(oracle, small, inp)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _oracle_step(oracle, small, inp)
+    dt = (time.perf_counter() - t0) / max(args.steps, 1)
+    tail, head = _flops(small)
+    v = 3 * (tail + head) / dt / 1e12
+    sample = "each step: first %d of %d tail groups (%d labels) + %d head labels of config 3 at B=%d" % (ng, cfg.NG, small.L_t, small.L_h, cfg.B)
+    print(json.dumps({
+        "impl": "reference", "metric": "sparse_layer_fwd_bwd_tflops_670k", "value": v, "unit": "TFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config3_670k_sample", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": "TFLOP/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="haste", choices=["haste", "reference"])
+    ap.add_argument("--workload", default=WORKLOAD, help="synth.CONFIGS key (default: the 670K-label config the metric is quoted on)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-head", action="store_true", help="time the sparse tail alone")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "haste" else args.warmup
+
+    from paper_2606_01117_b200 import synth
+    cfg = synth.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    from paper_2606_01117_b200 import haste     # fails loudly if libhaste.so is missing: no fallback
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- synthetic inputs of the workload's shape; replicas use their own seed
+    inp = synth.make_inputs(cfg, with_head=not args.no_head)
+    B, d, L, G, K, Lh = cfg.B, cfg.d, cfg.L_t, cfg.G, cfg.K, cfg.L_h
+    use_head = (not args.no_head) and Lh > 0
+
+    def bf(bits):
+        return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+
+    hX, hrow, hcol = bf(inp.bits["X"]).pin_memory(), torch.from_numpy(inp.rowptr).pin_memory(), torch.from_numpy(inp.col).pin_memory()
+    X, rowptr, col = hX.to(dev), hrow.to(dev), hcol.to(dev)
+    W, idx = bf(inp.bits["W"]).to(dev), torch.from_numpy(inp.idx).to(dev)
+    layer = haste.HasteLayer(d, L, G, K, B, "bf16", label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT, device=local)
+    layer.validate_index(idx)
+    dY = layer.alloc_dy(B)
+    dW = torch.empty(L, K, dtype=torch.bfloat16, device=dev)
+    db = torch.empty(L, device=dev)
+    dX = torch.empty(B, d, device=dev)
+    loss = torch.zeros(2, device=dev)
+    if use_head:
+        hXh = bf(inp.bits["X_head"]).pin_memory()
+        Xh, Wh = hXh.to(dev), bf(inp.bits["W_head"]).to(dev)
+        head = haste.HasteHead(d, Lh, B, "bf16", label_offset=0, device=local)
+        dYh = torch.empty(B, Lh, dtype=torch.bfloat16, device=dev)
+        dWh = torch.empty(Lh, d, dtype=torch.bfloat16, device=dev)
+        dbh = torch.empty(Lh, device=dev)
+        dXh = torch.empty(B, d, device=dev)
+    h_loss = torch.zeros(2).pin_memory()
+    h_dX = torch.empty(B, d).pin_memory()
+    h_dXh = torch.empty(B, d).pin_memory()
+    launches = [0]
+
+    def step():
+        n = 0
+        layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY)
+        n += layer.last_launch_count
+        layer.backward(B, X, idx, W, dY, dW=dW, dbias=db, dX=dX)
+        n += layer.last_launch_count
+        if use_head:
+            head.forward_loss(B, Xh, Wh, None, rowptr, col, loss=loss[1:2], dY=dYh)
+            n += head.last_launch_count
+            head.backward(B, Xh, Wh, dYh, dWh=dWh, dbias=dbh, dX=dXh)
+            n += head.last_launch_count
+        launches[0] += n
+
+    def step_e2e():
+        X.copy_(hX, non_blocking=True)
+        rowptr.copy_(hrow, non_blocking=True)
+        col.copy_(hcol, non_blocking=True)
+        if use_head:
+            Xh.copy_(hXh, non_blocking=True)
+        step()
+        h_loss.copy_(loss, non_blocking=True)
+        h_dX.copy_(dX, non_blocking=True)
+        if use_head:
+            h_dXh.copy_(dXh, non_blocking=True)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    layer.set_profiling(args.steps)
+    if use_head:
+        head.set_profiling(args.steps)
+    launches[0] = 0
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ms_total = timed(step, args.steps)
+    clocks = sampler.stop() if rank == 0 else None
+    n_launch = launches[0]
+    # per-kernel device times of the timed region (CUDA events recorded inside the library, on the launch stream)
+    kn = {"forward": haste.KERNEL_FORWARD, "dW": haste.KERNEL_DW, "dX": haste.KERNEL_DX,
+          "prep_fwd": haste.KERNEL_PREP_FWD, "prep_bwd": haste.KERNEL_PREP_BWD, "post_bwd": haste.KERNEL_POST_BWD}
+    kms = {k: [layer.kernel_ms(v, a) for a in range(args.steps)] for k, v in kn.items()}
+    if use_head:
+        kms["head_forward"] = [head.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(args.steps)]
+        kms["head_backward"] = [head.kernel_ms(haste.KERNEL_DW, a) for a in range(args.steps)]
+    layer.set_profiling(0)
+    if use_head:
+        head.set_profiling(0)
+    for _ in range(2):
+        step_e2e()
+    ms_e2e = timed(step_e2e, args.steps)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    peaks = _peaks()
+    tail_f, head_f = _flops(cfg)
+    step_flops = 3 * tail_f + (3 * head_f if use_head else 0)
+    ms_step = ms_total / args.steps
+    value = world * step_flops / (ms_step * 1e-3) / 1e12
+    e2e_value = world * step_flops / (ms_e2e / args.steps * 1e-3) / 1e12
+    ab = _alg_bytes(cfg)
+    kernels = {}
+    for k in ("forward", "dW", "dX"):
+        mean = float(np.mean(kms[k]))
+        gbs = ab[k] / (mean * 1e-3) / 1e9
+        kernels[k] = {"ms": mean, "ms_min": float(np.min(kms[k])), "GB/s": gbs, "frac_hbm": gbs / peaks["hbm"],
+                      "TFLOP/s": tail_f / (mean * 1e-3) / 1e12, "alg_bytes": ab[k]}
+    for k in kms:
+        if k not in kernels:
+            kernels[k] = {"ms": float(np.mean(kms[k])), "ms_min": float(np.min(kms[k]))}
+    if use_head:
+        kernels["head_forward"]["TFLOP/s"] = head_f / (kernels["head_forward"]["ms"] * 1e-3) / 1e12
+        kernels["head_backward"]["TFLOP/s"] = 2 * head_f / (kernels["head_backward"]["ms"] * 1e-3) / 1e12
+    dom = max(("forward", "dW", "dX"), key=lambda k: kernels[k]["ms"])
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["GB/s"], "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": kernels[dom]["GB/s"] / peaks["hbm"], "traffic": None, "peak_source": peaks["source"] + " (burst copy)",
+                "share_of_step": kernels[dom]["ms"] / ms_step}
+    h2d = hX.numel() * 2 + hrow.numel() * 4 + hcol.numel() * 4 + (hXh.numel() * 2 if use_head else 0)
+    d2h = 8 + B * d * 4 * (2 if use_head else 1)
+    out = {
+        "metric": "sparse_layer_fwd_bwd_tflops_670k", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "config3_670k" if args.workload == "670k" else args.workload, "B": B, "d": d, "L_tail": L, "L_head": Lh if use_head else 0,
+                   "G": G, "K": K, "replicas": world, "l2": "inputs larger than L2 (per pass W %d MB + dY %d MB vs 126 MB L2); no explicit flush" % (L * K * 2 >> 20, cfg.NG * G * B * 2 >> 20),
+                   "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}},
+        "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": int(n_launch), "clocks": clocks, "roofline": roofline, "kernels": kernels,
+        "loss": [float(v) for v in loss.cpu().tolist()],
+    }
+    if not args.no_cpu_baseline and world == 1:
+        out["cpu_baseline"] = cpu_baseline(cfg)
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

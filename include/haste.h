@@ -158,6 +158,26 @@ int haste_head_kernel_family(const haste_head_t* h);
 int haste_last_launch_count(const haste_layer_t* h);
 int haste_head_last_launch_count(const haste_head_t* h);
 
+/* Per-kernel device timing (measurement support).  haste_set_profiling(h, depth)
+ * with depth > 0 makes every forward / backward call record CUDA events on the caller's stream
+ * around its kernels and keeps the last `depth` calls (depth = 0 turns it off; the default).
+ * haste_kernel_ms waits for the events of one recorded run of `kernel` -- age 0 is the most recent
+ * run, age 1 the one before ... -- and returns its duration in milliseconds
+ * (HASTE_ERR_INVALID_ARG if no such run is held). */
+typedef enum {
+  HASTE_KERNEL_FORWARD = 0, /* forward contraction + fused BCE epilogue */
+  HASTE_KERNEL_DW = 1,      /* weight gradient                            */
+  HASTE_KERNEL_DX = 2,      /* input gradient scatter-add                    */
+  HASTE_KERNEL_PREP_FWD = 3,/* X -> X^T before the forward                                  */
+  HASTE_KERNEL_PREP_BWD = 4,/* X -> X^T and dX^T clear before the backward                  */
+  HASTE_KERNEL_POST_BWD = 5 /* dX^T -> dX                                                   */
+} haste_kernel_t;
+int haste_set_profiling(haste_layer_t* h, int depth);
+int haste_kernel_ms(haste_layer_t* h, int kernel /* haste_kernel_t */, int age, float* ms);
+int haste_head_set_profiling(haste_head_t* h, int depth);
+/* head kernels: HASTE_KERNEL_FORWARD, and HASTE_KERNEL_DW = the whole backward (dW_h, db, dX_h) */
+int haste_head_kernel_ms(haste_head_t* h, int kernel, int age, float* ms);
+
 #ifdef __cplusplus
 }
 #endif

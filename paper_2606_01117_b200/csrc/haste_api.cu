@@ -3,6 +3,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 #include <new>
 
 #include "kernels.h"
@@ -28,6 +29,49 @@ struct DeviceGuard {
   ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
+// Optional per-kernel device timing: CUDA events on the caller's stream around each main kernel,
+// kept in a ring of `depth` calls per kernel so a benchmark can read a whole timed region afterwards.
+struct Profiler {
+  static const int NSLOT = 6;
+  int depth = 0;
+  std::vector<cudaEvent_t> a[NSLOT], b[NSLOT];
+  long count[NSLOT] = {};     // completed begin/end pairs per slot
+  int enable(int new_depth) {
+    if (new_depth < 0 || new_depth > 4096) return HASTE_ERR_INVALID_ARG;
+    destroy();
+    for (int s = 0; s < NSLOT && new_depth > 0; ++s) {
+      a[s].assign(new_depth, nullptr);
+      b[s].assign(new_depth, nullptr);
+      for (int i = 0; i < new_depth; ++i)
+        if (cudaEventCreate(&a[s][i]) != cudaSuccess || cudaEventCreate(&b[s][i]) != cudaSuccess) return HASTE_ERR_CUDA;
+    }
+    depth = new_depth;
+    return HASTE_OK;
+  }
+  void begin(int s, cudaStream_t st) { if (depth) cudaEventRecord(a[s][count[s] % depth], st); }
+  void end(int s, cudaStream_t st) { if (depth) { cudaEventRecord(b[s][count[s] % depth], st); ++count[s]; } }
+  int ms(int s, int age, float* out) {
+    if (s < 0 || s >= NSLOT || !out || !depth || age < 0 || age >= depth || age >= count[s]) {
+      set_error("kernel_ms: profiling is off, or no such recorded call (kernel %d, age %d)", s, age);
+      return HASTE_ERR_INVALID_ARG;
+    }
+    const long i = (count[s] - 1 - age) % depth;
+    if (cudaEventSynchronize(b[s][i]) != cudaSuccess || cudaEventElapsedTime(out, a[s][i], b[s][i]) != cudaSuccess) {
+      set_error("kernel_ms: %s", cudaGetErrorString(cudaGetLastError()));
+      return HASTE_ERR_CUDA;
+    }
+    return HASTE_OK;
+  }
+  void destroy() {
+    for (int s = 0; s < NSLOT; ++s) {
+      for (cudaEvent_t e : a[s]) if (e) cudaEventDestroy(e);
+      for (cudaEvent_t e : b[s]) if (e) cudaEventDestroy(e);
+      a[s].clear(); b[s].clear(); count[s] = 0;
+    }
+    depth = 0;
+  }
+};
+
 static inline size_t esize(haste_dtype_t dt) { return dt == HASTE_F32 ? 4 : 2; }
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -49,6 +93,7 @@ struct haste_layer {
   int* flag;        // validate_index result
   TcTailState* tc;  // tcgen05 family state (tensor maps, counters) or NULL
   int last_launches;
+  Profiler* prof;
 };
 
 struct haste_head {
@@ -66,6 +111,7 @@ struct haste_head {
   int n_partials;
   TcHeadState* tc;
   int last_launches;
+  Profiler* prof;
 };
 
 extern "C" {
@@ -120,6 +166,8 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
   h->cfg = *cfg;
   h->device = cuda_device;
   h->NG = NG;
+  h->prof = new (std::nothrow) Profiler();
+  if (!h->prof) { delete h; return HASTE_ERR_NOMEM; }
   h->Bpad = round_up(cfg->B_max, 128);
   h->n_partials = 1024;
   const size_t xt_bytes = (size_t)cfg->d * h->Bpad * esize(cfg->dtype);
@@ -150,6 +198,7 @@ int haste_destroy(haste_layer_t* h) {
   if (!h) return HASTE_OK;
   DeviceGuard guard(h->device);
   if (h->tc) tc_tail_destroy(h->tc);
+  if (h->prof) { h->prof->destroy(); delete h->prof; }
   cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag);
   delete h;
   return HASTE_OK;
@@ -210,19 +259,24 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
   DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
   const TailShape sh = make_shape(h, B);
+  Profiler& pf = *h->prof;
   h->last_launches = 0;
   if (B == 0 || h->NG == 0) {
     if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(loss, 0, sizeof(float), st));
     return HASTE_OK;
   }
+  pf.begin(HASTE_KERNEL_PREP_FWD, st);
   rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
   if (rc) return rc;
   h->last_launches++;
+  pf.end(HASTE_KERNEL_PREP_FWD, st);
   if (h->family == 1) {
     int n = 0;
+    pf.begin(HASTE_KERNEL_FORWARD, st);
     rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY,
                          logits_out, st, &n);
     if (rc) return rc;
+    pf.end(HASTE_KERNEL_FORWARD, st);
     h->last_launches += n;
     if (loss) {
       rc = launch_finalize_loss(nullptr, h->partials, tc_tail_num_partials(h->tc), sh.s, loss, st);
@@ -232,9 +286,11 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
     return HASTE_OK;
   }
   if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(h->loss_acc, 0, sizeof(double), st));
+  pf.begin(HASTE_KERNEL_FORWARD, st);
   rc = launch_simt_forward(h->cfg.dtype, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->loss_acc : nullptr, dY,
                            logits_out, st);
   if (rc) return rc;
+  pf.end(HASTE_KERNEL_FORWARD, st);
   h->last_launches++;
   if (loss) {
     rc = launch_finalize_loss(h->loss_acc, nullptr, 0, sh.s, loss, st);
@@ -256,6 +312,7 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
   DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
   const TailShape sh = make_shape(h, B);
+  Profiler& pf = *h->prof;
   h->last_launches = 0;
   if (B == 0 || h->NG == 0) {
     if (dW && h->cfg.L > 0)
@@ -265,33 +322,57 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
     return HASTE_OK;
   }
   // The gather operand X^T is rebuilt here: backward must not depend on which forward ran last.
-  rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
-  if (rc) return rc;
-  h->last_launches++;
-  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
-  if (h->family == 1) {
-    int n = 0;
-    rc = tc_tail_backward(h->tc, sh, h->Xt, idx, W, dY, dW, dbias, dX ? h->dXt : nullptr, st, &n);
-    if (rc) return rc;
-    h->last_launches += n;
-  } else {
-    if (dW || dbias) {
-      rc = launch_simt_dw(h->cfg.dtype, h->cfg.dw_dtype, sh, h->Xt, idx, dY, dW, dbias, st);
-      if (rc) return rc;
-      h->last_launches++;
-    }
-    if (dX) {
-      rc = launch_simt_dx(h->cfg.dtype, sh, idx, W, dY, h->dXt, st);
-      if (rc) return rc;
-      h->last_launches++;
-    }
-  }
-  if (dX) {
-    rc = launch_untranspose_f32(h->dXt, dX, B, sh.d, h->Bpad, accumulate_dX, st);
+  pf.begin(HASTE_KERNEL_PREP_BWD, st);
+  if (dW || dbias) {
+    rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
     if (rc) return rc;
     h->last_launches++;
   }
+  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+  pf.end(HASTE_KERNEL_PREP_BWD, st);
+  if (dW || dbias) {
+    pf.begin(HASTE_KERNEL_DW, st);
+    if (h->family == 1) {
+      int n = 0;
+      rc = tc_tail_dw(h->tc, sh, h->Xt, idx, dY, dW, dbias, st, &n);
+      h->last_launches += n;
+    } else {
+      rc = launch_simt_dw(h->cfg.dtype, h->cfg.dw_dtype, sh, h->Xt, idx, dY, dW, dbias, st);
+      h->last_launches++;
+    }
+    if (rc) return rc;
+    pf.end(HASTE_KERNEL_DW, st);
+  }
+  if (dX) {
+    pf.begin(HASTE_KERNEL_DX, st);
+    if (h->family == 1) {
+      int n = 0;
+      rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, st, &n);
+      h->last_launches += n;
+    } else {
+      rc = launch_simt_dx(h->cfg.dtype, sh, idx, W, dY, h->dXt, st);
+      h->last_launches++;
+    }
+    if (rc) return rc;
+    pf.end(HASTE_KERNEL_DX, st);
+    pf.begin(HASTE_KERNEL_POST_BWD, st);
+    rc = launch_untranspose_f32(h->dXt, dX, B, sh.d, h->Bpad, accumulate_dX, st);
+    if (rc) return rc;
+    h->last_launches++;
+    pf.end(HASTE_KERNEL_POST_BWD, st);
+  }
   return HASTE_OK;
+}
+
+int haste_set_profiling(haste_layer_t* h, int depth) {
+  if (!h) { set_error("haste_set_profiling: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  return h->prof->enable(depth);
+}
+int haste_kernel_ms(haste_layer_t* h, int kernel, int age, float* ms) {
+  if (!h) { set_error("haste_kernel_ms: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  return h->prof->ms(kernel, age, ms);
 }
 
 int haste_dy_unpack(const haste_layer_t* h, int B, const void* dY, float* out_BL, void* stream) {
@@ -334,6 +415,8 @@ int haste_head_create(haste_head_t** out, int32_t d, int64_t L_h, int32_t B_max,
   h->d = d; h->L = L_h; h->B_max = B_max; h->dtype = dtype; h->label_offset = label_offset;
   h->loss_scale = loss_scale; h->flags = flags; h->device = cuda_device;
   h->n_partials = 1024;
+  h->prof = new (std::nothrow) Profiler();
+  if (!h->prof) { delete h; return HASTE_ERR_NOMEM; }
   cudaError_t e = cudaMalloc(&h->loss_acc, sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&h->partials, h->n_partials * sizeof(float));
   if (e == cudaSuccess) e = cudaMemset(h->partials, 0, h->n_partials * sizeof(float));
@@ -356,6 +439,7 @@ int haste_head_destroy(haste_head_t* h) {
   if (!h) return HASTE_OK;
   DeviceGuard guard(h->device);
   if (h->tc) tc_head_destroy(h->tc);
+  if (h->prof) { h->prof->destroy(); delete h->prof; }
   cudaFree(h->loss_acc); cudaFree(h->partials);
   delete h;
   return HASTE_OK;
@@ -388,6 +472,7 @@ int haste_head_forward_loss(haste_head_t* h, int B, const void* X, const void* W
   DeviceGuard guard(h->device);
   cudaStream_t st = (cudaStream_t)stream;
   const HeadShape sh = make_head_shape(h, B);
+  Profiler& pf = *h->prof;
   h->last_launches = 0;
   if (B == 0 || h->L == 0) {
     if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(loss, 0, sizeof(float), st));
@@ -396,8 +481,10 @@ int haste_head_forward_loss(haste_head_t* h, int B, const void* X, const void* W
   int rc;
   if (h->family == 1) {
     int n = 0;
+    pf.begin(HASTE_KERNEL_FORWARD, st);
     rc = tc_head_forward(h->tc, sh, X, Wh, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY, logits_out, st, &n);
     if (rc) return rc;
+    pf.end(HASTE_KERNEL_FORWARD, st);
     h->last_launches += n;
     if (loss) {
       rc = launch_finalize_loss(nullptr, h->partials, tc_head_num_partials(h->tc), sh.s, loss, st);
@@ -407,9 +494,11 @@ int haste_head_forward_loss(haste_head_t* h, int B, const void* X, const void* W
     return HASTE_OK;
   }
   if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(h->loss_acc, 0, sizeof(double), st));
+  pf.begin(HASTE_KERNEL_FORWARD, st);
   rc = launch_simt_head_forward(h->dtype, sh, X, Wh, bias, tgt_rowptr, tgt_col, loss ? h->loss_acc : nullptr, dY,
                                 logits_out, st);
   if (rc) return rc;
+  pf.end(HASTE_KERNEL_FORWARD, st);
   h->last_launches++;
   if (loss) {
     rc = launch_finalize_loss(h->loss_acc, nullptr, 0, sh.s, loss, st);
@@ -438,17 +527,31 @@ int haste_head_backward(haste_head_t* h, int B, const void* X, const void* Wh, c
     if (dX && !accumulate_dX && B > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dX, 0, (size_t)B * h->d * 4, st));
     return HASTE_OK;
   }
+  Profiler& pf = *h->prof;
+  pf.begin(HASTE_KERNEL_DW, st);     // the head's backward is timed as one unit (dW, db and dX)
   if (h->family == 1) {
     int n = 0;
     int rc = tc_head_backward(h->tc, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, st, &n);
     if (rc) return rc;
     h->last_launches += n;
-    return HASTE_OK;
+  } else {
+    int rc = launch_simt_head_backward(h->dtype, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, st);
+    if (rc) return rc;
+    h->last_launches += (dWh ? 1 : 0) + (dX ? 1 : 0) + (dbias ? 1 : 0);
   }
-  int rc = launch_simt_head_backward(h->dtype, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, st);
-  if (rc) return rc;
-  h->last_launches += (dWh ? 1 : 0) + (dX ? 1 : 0) + (dbias ? 1 : 0);
+  pf.end(HASTE_KERNEL_DW, st);
   return HASTE_OK;
+}
+
+int haste_head_set_profiling(haste_head_t* h, int depth) {
+  if (!h) { set_error("haste_head_set_profiling: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  return h->prof->enable(depth);
+}
+int haste_head_kernel_ms(haste_head_t* h, int kernel, int age, float* ms) {
+  if (!h) { set_error("haste_head_kernel_ms: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  return h->prof->ms(kernel, age, ms);
 }
 
 }  // extern "C"

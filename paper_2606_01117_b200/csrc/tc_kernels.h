@@ -18,8 +18,10 @@ int tc_tail_num_partials(const TcTailState* s);
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
                     const float* bias, const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY,
                     float* logits_out, cudaStream_t st, int* n_launches);
-int tc_tail_backward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
-                     const void* dY, void* dW, float* dbias, float* dXt, cudaStream_t st, int* n_launches);
+int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
+               float* dbias, cudaStream_t st, int* n_launches);
+int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
+               cudaStream_t st, int* n_launches);
 
 bool tc_head_supported(int d, int64_t L_h, int B_max, haste_dtype_t dtype, int device);
 int tc_head_create(TcHeadState** out, int d, int64_t L_h, int B_max, int device);

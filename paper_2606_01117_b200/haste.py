@@ -24,7 +24,9 @@ SYMBOLS = [
     "haste_backward", "haste_dy_unpack", "haste_dy_pack", "haste_head_create", "haste_head_destroy",
     "haste_head_forward_loss", "haste_head_backward", "haste_status_string", "haste_last_error",
     "haste_kernel_family", "haste_head_kernel_family", "haste_last_launch_count", "haste_head_last_launch_count",
+    "haste_set_profiling", "haste_kernel_ms", "haste_head_set_profiling", "haste_head_kernel_ms",
 ]
+KERNEL_FORWARD, KERNEL_DW, KERNEL_DX, KERNEL_PREP_FWD, KERNEL_PREP_BWD, KERNEL_POST_BWD = range(6)
 
 
 class haste_config_t(ctypes.Structure):
@@ -72,6 +74,10 @@ def lib():
     L.haste_last_error.restype = ctypes.c_char_p
     for n in ("haste_kernel_family", "haste_head_kernel_family", "haste_last_launch_count", "haste_head_last_launch_count"):
         getattr(L, n).argtypes = [vp]
+    for n in ("haste_set_profiling", "haste_head_set_profiling"):
+        getattr(L, n).argtypes = [vp, i32]
+    for n in ("haste_kernel_ms", "haste_head_kernel_ms"):
+        getattr(L, n).argtypes = [vp, i32, i32, ctypes.POINTER(f32)]
     _lib = L
     return L
 
@@ -132,6 +138,14 @@ class HasteLayer:
     def last_launch_count(self):
         return lib().haste_last_launch_count(self.h)
 
+    def set_profiling(self, depth=1):
+        _check(lib().haste_set_profiling(self.h, int(depth)))
+
+    def kernel_ms(self, kernel, age=0):
+        ms = ctypes.c_float()
+        _check(lib().haste_kernel_ms(self.h, kernel, age, ctypes.byref(ms)))
+        return ms.value
+
     def dy_bytes(self, B):
         return lib().haste_dy_bytes(self.h, B)
 
@@ -182,6 +196,14 @@ class HasteHead:
     @property
     def last_launch_count(self):
         return lib().haste_head_last_launch_count(self.h)
+
+    def set_profiling(self, depth=1):
+        _check(lib().haste_head_set_profiling(self.h, int(depth)))
+
+    def kernel_ms(self, kernel, age=0):
+        ms = ctypes.c_float()
+        _check(lib().haste_head_kernel_ms(self.h, kernel, age, ctypes.byref(ms)))
+        return ms.value
 
     def forward_loss(self, B, X, Wh, bias, rowptr, col, loss=None, dY=None, logits_out=None, stream=None):
         _check(lib().haste_head_forward_loss(self.h, B, _ptr(X), _ptr(Wh), _ptr(bias), _ptr(rowptr), _ptr(col),

@@ -1,0 +1,88 @@
+"""-m gpu parity of the dense head (haste_head_forward_loss / haste_head_backward)
+against the fp64 oracle."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_01117_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _case(seed, B, d, Lh, dtype, with_bias, n_pos=4, w_std=0.05, L_total=None):
+    X = synth.normal(seed, synth.STREAM_XHEAD, B * d).astype(np.float32).reshape(B, d)
+    W = (synth.normal(seed, synth.STREAM_WHEAD, Lh * d) * w_std).astype(np.float32).reshape(Lh, d)
+    bits = {}
+    if dtype == "bf16":
+        bits["X"], X = synth.round_bf16(X)
+        bits["W"], W = synth.round_bf16(W)
+        X, W = X.reshape(B, d), W.reshape(Lh, d)
+        bits["X"], bits["W"] = bits["X"].reshape(B, d), bits["W"].reshape(Lh, d)
+    bias = (synth.normal(seed, synth.STREAM_BIAS_HEAD, Lh) * 0.1).astype(np.float32) if with_bias else None
+    rowptr, col = synth.draw_targets(seed, B, L_total or Lh, 0, n_pos, None, n_fixed=min(n_pos, Lh))
+    return X, W, bias, rowptr, col, bits
+
+
+def _dev(a, bits=None):
+    dev = torch.device("cuda:0")
+    if a is None:
+        return None
+    if bits is not None:
+        return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).to(dev).view(torch.bfloat16)
+    return torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+
+HEAD_CASES = [
+    (32, 128, 300, "f32", True), (7, 40, 50, "f32", False),
+    (64, 128, 256, "bf16", True), (130, 256, 1000, "bf16", False), (256, 768, 4096, "bf16", True),
+    (512, 768, 2048 + 24, "bf16", False), (100, 200, 77, "bf16", True),
+]
+
+
+@pytest.mark.parametrize("force_simt", [False, True])
+@pytest.mark.parametrize("case", HEAD_CASES, ids=lambda c: "B%d_d%d_L%d_%s" % c[:4])
+def test_head_parity(oracle, case, force_simt):
+    from paper_2606_01117_b200 import haste
+    B, d, Lh, dt, with_bias = case
+    tol = 1e-5 if dt == "f32" else 5e-3
+    X, W, bias, rowptr, col, bits = _case(41 + B, B, d, Lh, dt, with_bias, L_total=Lh + 100)
+    dev = torch.device("cuda:0")
+    head = haste.HasteHead(d, Lh, B, dt, flags=haste.HASTE_FORCE_SIMT if force_simt else 0)
+    Xd, Wd = _dev(X, bits.get("X")), _dev(W, bits.get("W"))
+    bd, rp, cl = _dev(bias), _dev(rowptr), _dev(col)
+    loss = torch.full((1,), float("nan"), device=dev)
+    dY = torch.full((B, Lh), float("nan"), dtype=head.tdtype, device=dev)
+    z = torch.full((B, Lh), float("nan"), device=dev)
+    head.forward_loss(B, Xd, Wd, bd, rp, cl, loss=loss, dY=dY, logits_out=z)
+    assert head.last_launch_count > 0
+    ref = oracle.head_forward(X, W, bias, rowptr, col)
+    assert abs(loss.item() - ref["loss"]) <= tol * abs(ref["loss"])
+    assert oracle.rel_l2(z.cpu().numpy(), ref["z"]) <= 1e-5
+    dYn = dY.float().cpu().numpy()
+    assert np.all(np.isfinite(dYn))
+    assert oracle.rel_l2(dYn, ref["dY"]) <= tol
+    rows = np.repeat(np.arange(B), np.diff(rowptr))
+    keep = col < Lh
+    assert keep.any() and not keep.all()
+    assert oracle.rel_l2(dYn[rows[keep], col[keep]], ref["dY"][rows[keep], col[keep]]) <= tol
+    dW = torch.full((Lh, d), float("nan"), dtype=head.tdtype, device=dev)
+    db = torch.full((Lh,), float("nan"), device=dev)
+    dX = torch.full((B, d), float("nan"), device=dev)
+    head.backward(B, Xd, Wd, dY, dWh=dW, dbias=db, dX=dX)
+    bref = oracle.head_backward(X, W, ref["dY"])
+    assert oracle.rel_l2(dW.float().cpu().numpy(), bref["dW"]) <= tol
+    assert oracle.rel_l2(db.cpu().numpy(), bref["db"]) <= tol
+    assert oracle.rel_l2(dX.cpu().numpy(), bref["dX"]) <= tol
+    # accumulate_dX adds to the existing contents
+    dX2 = torch.ones(B, d, device=dev)
+    head.backward(B, Xd, Wd, dY, dWh=None, dbias=None, dX=dX2, accumulate_dX=True)
+    assert oracle.rel_l2(dX2.cpu().numpy() - 1.0, bref["dX"]) <= max(tol, 1e-4)
+
+
+def test_head_empty():
+    from paper_2606_01117_b200 import haste
+    dev = torch.device("cuda:0")
+    head = haste.HasteHead(16, 0, 8, "f32")
+    loss = torch.full((1,), 3.0, device=dev)
+    head.forward_loss(8, torch.zeros(8, 16, device=dev), torch.zeros(1, 16, device=dev), None, None, None, loss=loss)
+    assert loss.item() == 0.0
