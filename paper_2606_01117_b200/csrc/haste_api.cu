@@ -332,11 +332,13 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
   pf.end(HASTE_KERNEL_PREP_BWD, st);
   if (dW || dbias) {
     pf.begin(HASTE_KERNEL_DW, st);
+    rc = HASTE_ERR_UNSUPPORTED;
     if (h->family == 1) {
       int n = 0;
       rc = tc_tail_dw(h->tc, sh, h->Xt, idx, dY, dW, dbias, st, &n);
-      h->last_launches += n;
-    } else {
+      if (rc == HASTE_OK) h->last_launches += n;
+    }
+    if (rc == HASTE_ERR_UNSUPPORTED) {   // shapes / outputs the tcgen05 dW kernel does not cover run the CUDA-core kernel
       rc = launch_simt_dw(h->cfg.dtype, h->cfg.dw_dtype, sh, h->Xt, idx, dY, dW, dbias, st);
       h->last_launches++;
     }
@@ -345,11 +347,13 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
   }
   if (dX) {
     pf.begin(HASTE_KERNEL_DX, st);
+    rc = HASTE_ERR_UNSUPPORTED;
     if (h->family == 1) {
       int n = 0;
       rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, st, &n);
-      h->last_launches += n;
-    } else {
+      if (rc == HASTE_OK) h->last_launches += n;
+    }
+    if (rc == HASTE_ERR_UNSUPPORTED) {
       rc = launch_simt_dx(h->cfg.dtype, sh, idx, W, dY, h->dXt, st);
       h->last_launches++;
     }

@@ -1,13 +1,472 @@
-// tc_tail.cu -- tcgen05 sparse-tail kernels (placeholder while the family is brought up).
+// tc_tail.cu -- tcgen05 / TMEM / TMA kernels of the HASTE sparse tail (sm_100a; bf16 in, fp32 accumulate).
+//
+// Forward + fused BCE (PAPER.md:97 "gather-once, dense GEMM per group", :111 Eq. 3):
+//   persistent CTAs, one per SM.  A CTA owns a pair of 128-row batch tiles and a stripe of groups.
+//   per (group g, batch tile): Z[128 x G] = H_g[128 x K] * W_g^T, H_g = X[:, idx_g] gathered from X^T.
+//   warp roles (448 threads):
+//     warps 0-7   epilogue: TMEM -> registers -> sigmoid/softplus (1 MUFU per logit) -> bf16 dY
+//                 -> swizzled smem tile -> TMA store; loss partial per thread.  Two halves of 4 warps
+//                 work on alternate tiles; a thread owns ONE batch row for the whole kernel, so its
+//                 CSR target row is walked once with a running cursor.
+//     warps 8-11  gather producers: cp.async 16-B chunks of X^T rows idx_g into the swizzled H image.
+//     warp 12     MMA issuer (one thread): tcgen05.mma M=128, N=G, K=16 x (K/16) into a TMEM slot ring.
+//     warp 13     TMA loader of W_g (the [G x K] block is contiguous in W).
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "tc_common.cuh"
 #include "tc_kernels.h"
+
 namespace haste {
-struct TcTailState { int dummy; };
-bool tc_tail_supported(const haste_config_t&, int) { return false; }
-int tc_tail_create(TcTailState**, const haste_config_t&, int, int) { return HASTE_ERR_UNSUPPORTED; }
-void tc_tail_destroy(TcTailState*) {}
-int tc_tail_num_partials(const TcTailState*) { return 0; }
-int tc_tail_forward(TcTailState*, const TailShape&, const void*, const int32_t*, const void*, const float*, const int32_t*,
-                    const int32_t*, float*, void*, float*, cudaStream_t, int*) { return HASTE_ERR_UNSUPPORTED; }
-int tc_tail_dw(TcTailState*, const TailShape&, const void*, const int32_t*, const void*, void*, float*, cudaStream_t, int*) { return HASTE_ERR_UNSUPPORTED; }
-int tc_tail_dx(TcTailState*, const TailShape&, const int32_t*, const void*, const void*, float*, cudaStream_t, int*) { return HASTE_ERR_UNSUPPORTED; }
+
+// ---------------------------------------------------------------------------------------------
+// host: tensor-map encoding through the driver entry point (no link-time libcuda dependency)
+// ---------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
 }
+
+int encode_tmap(CUtensorMap* out, int dtype_bytes, const void* base, int rank, const uint64_t* dims,
+                const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) { set_error("cuTensorMapEncodeTiled is not available from the driver"); return HASTE_ERR_CUDA; }
+  cuuint64_t gd[5]; cuuint64_t gs[4]; cuuint32_t bx[5]; cuuint32_t es[5];
+  for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; }
+  for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_bytes[i];
+  const CUtensorMapSwizzle sw = swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                              : swizzle_bytes == 64  ? CU_TENSOR_MAP_SWIZZLE_64B
+                              : swizzle_bytes == 32  ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE;
+  const CUtensorMapDataType dt = dtype_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  CUresult r = fn(out, dt, (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return HASTE_ERR_CUDA; }
+  return HASTE_OK;
+}
+
+using namespace tc;
+
+// ---------------------------------------------------------------------------------------------
+// forward
+// ---------------------------------------------------------------------------------------------
+struct FwdParams {
+  const bf16* Xt;          // [d][Bpad]
+  const int32_t* idx;      // [NG][K]
+  const float* bias;       // [L] or null
+  const int32_t* rowptr;   // [B+1] or null
+  const int32_t* col;      // [nnz]
+  float* partials;         // [gridDim.x] unscaled loss partials, or null
+  float* logits;           // [B][L] fp32 or null
+  int write_dy;
+  int B, Bpad, NT, NP, S;  // NT batch tiles of 128; NP tile pairs; S group stripes (grid = NP*S)
+  int64_t L, NG, label_offset;
+  float s;
+};
+
+template <int G, int K> struct FwdCfg {
+  static constexpr int HS = (G == 128 && K == 128) ? 3 : 4;     // H stages
+  static constexpr int LAG = 2;                                 // producer completion lag (<= HS-1)
+  static constexpr int H_BYTES = K * 256;                       // [2 m-blocks][K rows][128 B]
+  static constexpr int W_BYTES = G * K * 2;                     // [K/64 k-blocks][G rows][128 B]
+  static constexpr int ST_BYTES = 128 * G * 2;                  // one dY staging tile per epilogue half
+  static constexpr int NSLOT = (512 / G) >= 8 ? 8 : (512 / G);  // TMEM accumulator ring (G columns each)
+  static constexpr int OFF_H = 0;
+  static constexpr int OFF_W = OFF_H + HS * H_BYTES;
+  static constexpr int OFF_ST = OFF_W + 2 * W_BYTES;
+  static constexpr int OFF_BIAS = OFF_ST + 2 * ST_BYTES;
+  static constexpr int OFF_BAR = OFF_BIAS + 2 * G * 4;
+  static constexpr int NBAR = 2 * HS + 4 + 2 * NSLOT;
+  static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;           // tmem base, loss scratch
+  static constexpr int SMEM = OFF_MISC + 64 + 1024;             // + alignment slack
+};
+
+__device__ __forceinline__ float tanh_approx(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// 32 logits of one batch row: z -> dY (bf16x2 packed) and the row's loss terms.
+//   sigma(z) = 1/2 + 1/2 tanh(z/2)  (one MUFU op);  softplus(z) = max(z,0) - ln( sigma(|z|) ), and the
+//   logs of a tile are taken once on the PRODUCT of the factors sigma(|z|) in [1/2,1)  (<= 16 per chain).
+// SLOW: some label of this chunk is a positive of this row, or the chunk holds padding labels (>= L).
+template <bool SLOW, bool BIAS>
+__device__ __forceinline__ void epi32(const uint32_t (&v)[32], const float* sbias, uint32_t ymask, int nvalid, float s,
+                                      float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
+#pragma unroll
+  for (int j = 0; j < 32; j += 2) {
+    float dy[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int jj = j + u;
+      float z = __uint_as_float(v[jj]);
+      if (BIAS) z += sbias[jj];
+      const float t = tanh_approx(0.5f * z);
+      float d = fmaf(t, hs, hs);
+      float f = fmaf(fabsf(t), 0.5f, 0.5f);
+      float r = fmaxf(z, 0.f);
+      if (SLOW) {
+        const bool valid = jj < nvalid;
+        const bool y = (ymask >> jj) & 1u;
+        if (y) { d -= s; r -= z; }
+        if (!valid) { d = 0.f; f = 1.f; r = 0.f; }
+        if (zout && valid) zout[jj] = z;
+      }
+      dy[u] = d;
+      P[jj & 3] *= f;
+      R[jj & 3] += r;
+    }
+    out[j >> 1] = pack_bf16x2(dy[0], dy[1]);
+  }
+}
+
+template <int G, int K>
+__global__ void __launch_bounds__(448, 1)
+tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmY, const FwdParams p) {
+  using C = FwdCfg<G, K>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
+  uint64_t* h_full = bars;                       // [HS]  count 4 (producer warps)
+  uint64_t* h_empty = bars + C::HS;              // [HS]  count 1 (umma commit)
+  uint64_t* w_full = bars + 2 * C::HS;           // [2]   count 1 + tx
+  uint64_t* w_empty = w_full + 2;                // [2]   count 1 (umma commit)
+  uint64_t* t_full = w_empty + 2;                // [NSLOT] count 1 (umma commit)
+  uint64_t* t_empty = t_full + C::NSLOT;         // [NSLOT] count 4 (epilogue warps of one half)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
+  float* loss_red = reinterpret_cast<float*>(smem + C::OFF_MISC + 16);   // [8]
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int pr = blockIdx.x % p.NP, stripe = blockIdx.x / p.NP;
+  const int ntp = min(2, p.NT - 2 * pr);                                  // batch tiles of this CTA's pair
+  const int ngl = (int)((p.NG - stripe + p.S - 1) / p.S);                 // groups of this CTA's stripe
+  const int total = ngl * ntp;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < C::HS; ++i) { mbar_init(&h_full[i], 4); mbar_init(&h_empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&w_full[i], 1); mbar_init(&w_empty[i], 1); }
+    for (int i = 0; i < C::NSLOT; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
+    fence_barrier_init();
+  }
+  if (warp == 13 && lane == 0) { tma_prefetch_desc(&tmW); tma_prefetch_desc(&tmY); }
+  if (warp == 12) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp >= 8 && warp < 12) {
+    // ===================== gather producers =====================
+    const int pw = warp - 8;
+    constexpr int RPW = K / 4;                       // rows (slots) per producer warp
+    int myidx = 0;
+    const int sub = lane >> 4, c = lane & 15;        // two rows per instruction, 16 chunks of 16 B per row
+    const uint32_t dst_lane = (uint32_t)((c >> 3) * (K * 128) + (((c & 7)) << 4));
+    for (int T = 0; T < total; ++T) {
+      const int gl = T / ntp, which = T - gl * ntp;
+      if (which == 0) {
+        const int64_t g = stripe + (int64_t)gl * p.S;
+        myidx = (lane < RPW) ? __ldg(p.idx + g * K + pw * RPW + lane) : 0;
+      }
+      const int hs = T % C::HS;
+      mbar_wait(&h_empty[hs], ((T / C::HS) & 1) ^ 1);
+      const int b0 = (2 * pr + which) * 128;
+      const uint32_t dst0 = smem_u32(smem + C::OFF_H + hs * C::H_BYTES) + dst_lane;
+      const bf16* src0 = p.Xt + b0 + c * 8;
+#pragma unroll
+      for (int i = 0; i < RPW / 2; ++i) {
+        const int kk = 2 * i + sub;
+        const int f = __shfl_sync(0xffffffffu, myidx, kk);
+        const int k = pw * RPW + kk;
+        // row k of the image, chunk (c&7) XOR (k&7): the 128-byte swizzle of the UMMA / TMA layouts
+        const uint32_t dst = (dst0 + k * 128) ^ ((uint32_t)(k & 7) << 4);
+        cp_async16(dst, src0 + (size_t)f * p.Bpad);
+      }
+      cp_async_commit();
+      if (T >= C::LAG) {
+        cp_async_wait<C::LAG>();
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&h_full[(T - C::LAG) % C::HS]);
+      }
+    }
+    // drain the last LAG tiles
+#pragma unroll
+    for (int r = C::LAG - 1; r >= 0; --r) {
+      const int T = total - 1 - r;
+      if (T >= 0) {
+        if (r == 1) cp_async_wait<1>(); else cp_async_wait<0>();
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&h_full[T % C::HS]);
+      }
+    }
+  } else if (warp == 12) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = make_idesc_bf16(128, G, /*A MN-major*/ 1, /*B K-major*/ 0);
+      for (int T = 0; T < total; ++T) {
+        const int gl = T / ntp, which = T - gl * ntp;
+        const int ws = gl & 1, hs = T % C::HS, slot = T % C::NSLOT;
+        if (which == 0) mbar_wait(&w_full[ws], (gl >> 1) & 1);
+        mbar_wait(&h_full[hs], (T / C::HS) & 1);
+        mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t a0 = smem_u32(smem + C::OFF_H + hs * C::H_BYTES);
+        const uint32_t b0 = smem_u32(smem + C::OFF_W + ws * C::W_BYTES);
+        const uint32_t d = tmem_base + slot * G;
+#pragma unroll
+        for (int j = 0; j < K / 16; ++j) {
+          const uint64_t ad = make_sdesc_sw128(a0 + j * 2048, K * 128, 1024);
+          const uint64_t bd = make_sdesc_sw128(b0 + (j >> 2) * (G * 128) + (j & 3) * 32, 16, 1024);
+          umma_f16(d, ad, bd, idesc, j > 0 ? 1u : 0u);
+        }
+        umma_commit(&h_empty[hs]);
+        umma_commit(&t_full[slot]);
+        if (which == ntp - 1) umma_commit(&w_empty[ws]);
+      }
+    }
+  } else if (warp == 13) {
+    // ===================== W loader =====================
+    if (lane == 0) {
+      for (int gl = 0; gl < ngl; ++gl) {
+        const int ws = gl & 1;
+        const int64_t g = stripe + (int64_t)gl * p.S;
+        mbar_wait(&w_empty[ws], ((gl >> 1) & 1) ^ 1);
+        mbar_arrive_expect_tx(&w_full[ws], C::W_BYTES);
+#pragma unroll
+        for (int kb = 0; kb < K / 64; ++kb)
+          tma_load_2d(smem + C::OFF_W + ws * C::W_BYTES + kb * (G * 128), &tmW, &w_full[ws], kb * 64, (int)(g * G));
+      }
+    }
+  } else {
+    // ===================== epilogue =====================
+    const int half = warp >> 2, q = warp & 3;
+    const int tih = threadIdx.x & 127;                         // thread index inside the half
+    const int row = q * 32 + lane;                             // row of the batch tile == TMEM lane
+    const int my_bt = 2 * pr + (ntp == 2 ? half : 0);
+    const int b = my_bt * 128 + row;
+    const bool valid_row = b < p.B;
+    int pc = 0, pe = 0;
+    int nxt = 0x7fffffff;
+    if (valid_row && p.rowptr) {
+      pc = __ldg(p.rowptr + b); pe = __ldg(p.rowptr + b + 1);
+      if (pc < pe) nxt = __ldg(p.col + pc);
+    }
+    float loss_local = 0.f;
+    const float hs = 0.5f * p.s;
+    uint8_t* stage = smem + C::OFF_ST + half * C::ST_BYTES;
+    float* sbias = reinterpret_cast<float*>(smem + C::OFF_BIAS) + half * G;
+    const bool issuer = tih == 0;
+    for (int T = half; T < total; T += 2) {
+      const int gl = T / ntp;
+      const int64_t g = stripe + (int64_t)gl * p.S;
+      const int nl = (int)min((int64_t)G, p.L - g * G);
+      const int slot = T % C::NSLOT;
+      if (issuer) bulk_wait_read<0>();                         // the staging tile is free again
+      if (p.bias && tih < G) sbias[tih] = tih < nl ? __ldg(p.bias + g * G + tih) : 0.f;
+      named_bar_sync(1 + half, 128);
+      // positives of this row inside the group: walk the CSR cursor (ascending groups, fixed row)
+      const int64_t glo64 = p.label_offset + g * G;
+      const int glo = (int)min(glo64, (int64_t)0x7fffffff), ghi = (int)min(glo64 + nl, (int64_t)0x7fffffff);
+      uint32_t ym[G / 32];
+#pragma unroll
+      for (int i = 0; i < G / 32; ++i) ym[i] = 0;
+      while (nxt < ghi) {
+        if (nxt >= glo) {
+          const int o = nxt - glo;
+#pragma unroll
+          for (int i = 0; i < G / 32; ++i) if ((o >> 5) == i) ym[i] |= 1u << (o & 31);
+        }
+        ++pc;
+        nxt = pc < pe ? __ldg(p.col + pc) : 0x7fffffff;
+      }
+      uint32_t anyy = 0;
+#pragma unroll
+      for (int i = 0; i < G / 32; ++i) anyy |= ym[i];
+      const bool slow = __any_sync(0xffffffffu, anyy != 0) || nl < G || p.logits != nullptr;
+
+      mbar_wait(&t_full[slot], (T / C::NSLOT) & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * G;
+      float R[4] = {0.f, 0.f, 0.f, 0.f}, P[4] = {1.f, 1.f, 1.f, 1.f};
+      uint32_t v[2][32];
+      tmem_ld32(taddr, v[0]);
+#pragma unroll
+      for (int sc = 0; sc < G / 32; ++sc) {
+        tmem_ld_wait();
+        if (sc + 1 < G / 32) tmem_ld32(taddr + (sc + 1) * 32, v[(sc + 1) & 1]);
+        else {
+          // all of this warp's TMEM reads are done: hand the accumulator slot back to the MMA issuer
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&t_empty[slot]);
+        }
+        uint32_t out[16];
+        float* zout = (p.logits && valid_row) ? p.logits + (size_t)b * p.L + g * G + sc * 32 : nullptr;
+        const int nvalid = nl - sc * 32;
+        if (slow) {
+          if (p.bias) epi32<true, true>(v[sc & 1], sbias + sc * 32, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+          else epi32<true, false>(v[sc & 1], nullptr, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+        } else {
+          if (p.bias) epi32<false, true>(v[sc & 1], sbias + sc * 32, 0u, 32, p.s, hs, R, P, out, nullptr);
+          else epi32<false, false>(v[sc & 1], nullptr, 0u, 32, p.s, hs, R, P, out, nullptr);
+        }
+        if (sc & 1) {   // 64 factors in [1/2,1) at most per product: fold into the loss, restart the chains
+          loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { R[i] = 0.f; P[i] = 1.f; }
+        }
+        if (p.write_dy) {
+          if (G >= 64) {
+            uint8_t* rowp = stage + (sc >> 1) * 16384 + row * 128;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int ch = ((sc & 1) * 4 + i) ^ (row & 7);
+              *reinterpret_cast<uint4*>(rowp + ch * 16) = make_uint4(out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
+            }
+          } else {
+            uint8_t* rowp = stage + row * 64;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int ch = i ^ ((row >> 1) & 3);
+              *reinterpret_cast<uint4*>(rowp + ch * 16) = make_uint4(out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
+            }
+          }
+        }
+      }
+      if ((G / 32) & 1)
+        loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
+      if (p.write_dy) fence_proxy_async_smem();
+      named_bar_sync(1 + half, 128);
+      if (p.write_dy) {
+        if (issuer) {
+#pragma unroll
+          for (int sb = 0; sb < (G + 63) / 64; ++sb) tma_store_3d(&tmY, stage + sb * 16384, sb * 64, my_bt * 128, (int)g);
+          bulk_commit();
+        }
+      }
+    }
+    if (issuer) bulk_wait<0>();
+    if (!valid_row) loss_local = 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) loss_local += __shfl_xor_sync(0xffffffffu, loss_local, o);
+    if (lane == 0) loss_red[warp] = loss_local;
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 12) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
+  if (threadIdx.x == 0 && p.partials) {
+    float t = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) t += loss_red[i];
+    p.partials[blockIdx.x] = t;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+struct TcTailState {
+  haste_config_t cfg;
+  int device, num_sms, Bpad;
+  int n_partials;
+};
+
+bool tc_tail_supported(const haste_config_t& cfg, int) {
+  if (cfg.dtype != HASTE_BF16) return false;
+  if (!(cfg.G == 32 || cfg.G == 64 || cfg.G == 128)) return false;
+  if (!(cfg.K == 64 || cfg.K == 128)) return false;
+  if (cfg.L < 1 || cfg.B_max > 128 * 2 * 128) return false;
+  return true;
+}
+
+int tc_tail_create(TcTailState** out, const haste_config_t& cfg, int Bpad, int device) {
+  TcTailState* s = new (std::nothrow) TcTailState();
+  if (!s) return HASTE_ERR_NOMEM;
+  s->cfg = cfg; s->device = device; s->Bpad = Bpad;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete s; set_error("cudaGetDeviceProperties failed"); return HASTE_ERR_CUDA; }
+  if (prop.major != 10) { delete s; set_error("the tcgen05 kernel family needs an sm_100 device (found sm_%d%d)", prop.major, prop.minor); return HASTE_ERR_UNSUPPORTED; }
+  s->num_sms = prop.multiProcessorCount;
+  s->n_partials = s->num_sms;
+  if (!get_encode_fn()) { delete s; set_error("cuTensorMapEncodeTiled is not available from the driver"); return HASTE_ERR_CUDA; }
+  *out = s;
+  return HASTE_OK;
+}
+void tc_tail_destroy(TcTailState* s) { delete s; }
+int tc_tail_num_partials(const TcTailState* s) { return s->n_partials; }
+
+template <int G, int K>
+static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
+                      const int32_t* rowptr, const int32_t* col, float* partials, void* dY, float* logits, cudaStream_t st) {
+  using C = FwdCfg<G, K>;
+  static_assert(C::SMEM <= 232448, "shared memory budget");
+  CUtensorMap tmW, tmY;
+  {
+    const uint64_t dims[2] = {(uint64_t)K, (uint64_t)sh.L};
+    const uint64_t str[1] = {(uint64_t)K * 2};
+    const uint32_t box[2] = {64, (uint32_t)G};
+    int rc = encode_tmap(&tmW, 2, W, 2, dims, str, box, 128);
+    if (rc) return rc;
+  }
+  if (dY) {
+    const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
+    const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
+    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 128, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
+    if (rc) return rc;
+  } else {
+    tmY = tmW;
+  }
+  FwdParams p;
+  p.Xt = (const bf16*)Xt; p.idx = idx; p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = partials; p.logits = logits;
+  p.write_dy = dY ? 1 : 0;
+  p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NP = (p.NT + 1) / 2;
+  p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NP));
+  p.L = sh.L; p.NG = sh.NG; p.label_offset = sh.label_offset; p.s = sh.s;
+  if (p.NP > s->num_sms) { set_error("batch too large for the tcgen05 forward"); return HASTE_ERR_UNSUPPORTED; }
+  const int grid = p.NP * p.S;
+  if (partials && grid < s->n_partials)   // partials beyond the grid stay zero from create / earlier calls: clear them
+    HASTE_CUDA_TRY(cudaMemsetAsync(partials + grid, 0, (size_t)(s->n_partials - grid) * sizeof(float), st));
+  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+  tc_fwd_kernel<G, K><<<grid, 448, C::SMEM, st>>>(tmW, tmY, p);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
+                    const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
+                    cudaStream_t st, int* n_launches) {
+  *n_launches = 1;
+#define HASTE_FWD(G_, K_) \
+  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, dY, logits_out, st)
+  HASTE_FWD(64, 128); HASTE_FWD(64, 64); HASTE_FWD(32, 64); HASTE_FWD(32, 128); HASTE_FWD(128, 64); HASTE_FWD(128, 128);
+#undef HASTE_FWD
+  set_error("tcgen05 forward: unsupported (G, K)");
+  return HASTE_ERR_UNSUPPORTED;
+}
+
+int tc_tail_dw(TcTailState*, const TailShape&, const void*, const int32_t*, const void*, void*, float*, cudaStream_t, int*) {
+  return HASTE_ERR_UNSUPPORTED;
+}
+int tc_tail_dx(TcTailState*, const TailShape&, const int32_t*, const void*, const void*, float*, cudaStream_t, int*) {
+  return HASTE_ERR_UNSUPPORTED;
+}
+
+}  // namespace haste
