@@ -78,14 +78,15 @@ template <int G, int K> struct FwdCfg {
   static constexpr int LAG = 2;                                 // producer completion lag (<= HS-1)
   static constexpr int H_BYTES = K * 256;                       // [2 m-blocks][K rows][128 B]
   static constexpr int W_BYTES = G * K * 2;                     // [K/64 k-blocks][G rows][128 B]
-  static constexpr int ST_BYTES = 128 * G * 2;                  // one dY staging tile per epilogue half
+  static constexpr int WS = W_BYTES <= 16384 ? 3 : 2;           // W stages
+  static constexpr int ST_BYTES = 128 * (G < 64 ? G : 64) * 2;  // one dY staging tile (<= 64 labels wide) per epilogue half
   static constexpr int NSLOT = (512 / G) >= 8 ? 8 : (512 / G);  // TMEM accumulator ring (G columns each)
   static constexpr int OFF_H = 0;
   static constexpr int OFF_W = OFF_H + HS * H_BYTES;
-  static constexpr int OFF_ST = OFF_W + 2 * W_BYTES;
-  static constexpr int OFF_BIAS = OFF_ST + 2 * ST_BYTES;
-  static constexpr int OFF_BAR = OFF_BIAS + 2 * G * 4;
-  static constexpr int NBAR = 2 * HS + 4 + 2 * NSLOT;
+  static constexpr int OFF_ST = OFF_W + WS * W_BYTES;
+  static constexpr int OFF_BIAS = OFF_ST + 2 * ST_BYTES;        // [8 warps][G] fp32
+  static constexpr int OFF_BAR = OFF_BIAS + 8 * G * 4;
+  static constexpr int NBAR = 2 * HS + 2 * WS + 2 * NSLOT;
   static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;           // tmem base, loss scratch
   static constexpr int SMEM = OFF_MISC + 64 + 1024;             // + alignment slack
 };
@@ -105,16 +106,21 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 //   logs of a tile are taken once on the PRODUCT of the factors sigma(|z|) in [1/2,1)  (<= 16 per chain).
 // SLOW: some label of this chunk is a positive of this row, or the chunk holds padding labels (>= L).
 template <bool SLOW, bool BIAS>
-__device__ __forceinline__ void epi32(const uint32_t (&v)[32], const float* sbias, uint32_t ymask, int nvalid, float s,
+__device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
                                       float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
+  float bv[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
   for (int j = 0; j < 32; j += 2) {
     float dy[2];
+    if (BIAS && (j & 3) == 0) {
+      const float4 t4 = lds128f(sbias + j * 4);
+      bv[0] = t4.x; bv[1] = t4.y; bv[2] = t4.z; bv[3] = t4.w;
+    }
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
       const int jj = j + u;
       float z = __uint_as_float(v[jj]);
-      if (BIAS) z += sbias[jj];
+      if (BIAS) z += bv[jj & 3];
       const float t = tanh_approx(0.5f * z);
       float d = fmaf(t, hs, hs);
       float f = fmaf(fabsf(t), 0.5f, 0.5f);
@@ -140,25 +146,27 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   using C = FwdCfg<G, K>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t sbase = smem_u32(smem);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
   uint64_t* h_full = bars;                       // [HS]  count 4 (producer warps)
   uint64_t* h_empty = bars + C::HS;              // [HS]  count 1 (umma commit)
-  uint64_t* w_full = bars + 2 * C::HS;           // [2]   count 1 + tx
-  uint64_t* w_empty = w_full + 2;                // [2]   count 1 (umma commit)
-  uint64_t* t_full = w_empty + 2;                // [NSLOT] count 1 (umma commit)
+  uint64_t* w_full = bars + 2 * C::HS;           // [WS]  count 1 + tx
+  uint64_t* w_empty = w_full + C::WS;            // [WS]  count 1 (umma commit)
+  uint64_t* t_full = w_empty + C::WS;            // [NSLOT] count 1 (umma commit)
   uint64_t* t_empty = t_full + C::NSLOT;         // [NSLOT] count 4 (epilogue warps of one half)
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
   float* loss_red = reinterpret_cast<float*>(smem + C::OFF_MISC + 16);   // [8]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int pr = blockIdx.x % p.NP, stripe = blockIdx.x / p.NP;
-  const int ntp = min(2, p.NT - 2 * pr);                                  // batch tiles of this CTA's pair
+  const int ntp = min(2, p.NT - 2 * pr);                                  // batch tiles of this CTA's pair (1 or 2)
+  const int tsh = ntp - 1;                                                // T >> tsh = group, T & tsh = tile of the pair
   const int ngl = (int)((p.NG - stripe + p.S - 1) / p.S);                 // groups of this CTA's stripe
-  const int total = ngl * ntp;
+  const int total = ngl << tsh;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < C::HS; ++i) { mbar_init(&h_full[i], 4); mbar_init(&h_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&w_full[i], 1); mbar_init(&w_empty[i], 1); }
+    for (int i = 0; i < C::WS; ++i) { mbar_init(&w_full[i], 1); mbar_init(&w_empty[i], 1); }
     for (int i = 0; i < C::NSLOT; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
     fence_barrier_init();
   }
@@ -173,24 +181,31 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     // ===================== gather producers =====================
     const int pw = warp - 8;
     constexpr int RPW = K / 4;                       // rows (slots) per producer warp
-    int myidx = 0;
     const int sub = lane >> 4, c = lane & 15;        // two rows per instruction, 16 chunks of 16 B per row
     const uint32_t dst_lane = (uint32_t)((c >> 3) * (K * 128) + (((c & 7)) << 4));
+    const int32_t* idx_ptr = p.idx + (int64_t)stripe * K + pw * RPW + lane;   // this lane's slot of group gl: + gl*S*K
+    const int64_t idx_step = (int64_t)p.S * K;
+    // slot indices are prefetched two groups ahead so that the gather never waits on an HBM read of idx
+    int idx_cur = 0, idx_n1 = 0, idx_n2 = 0;
+    if (lane < RPW) {
+      idx_n1 = __ldg(idx_ptr);
+      if (ngl > 1) idx_n2 = __ldg(idx_ptr + idx_step);
+    }
     for (int T = 0; T < total; ++T) {
-      const int gl = T / ntp, which = T - gl * ntp;
+      const int gl = T >> tsh, which = T & tsh;
       if (which == 0) {
-        const int64_t g = stripe + (int64_t)gl * p.S;
-        myidx = (lane < RPW) ? __ldg(p.idx + g * K + pw * RPW + lane) : 0;
+        idx_cur = idx_n1; idx_n1 = idx_n2;
+        if (lane < RPW && gl + 2 < ngl) idx_n2 = __ldg(idx_ptr + (gl + 2) * idx_step);
       }
       const int hs = T % C::HS;
       mbar_wait(&h_empty[hs], ((T / C::HS) & 1) ^ 1);
       const int b0 = (2 * pr + which) * 128;
-      const uint32_t dst0 = smem_u32(smem + C::OFF_H + hs * C::H_BYTES) + dst_lane;
+      const uint32_t dst0 = sbase + C::OFF_H + hs * C::H_BYTES + dst_lane;
       const bf16* src0 = p.Xt + b0 + c * 8;
 #pragma unroll
       for (int i = 0; i < RPW / 2; ++i) {
         const int kk = 2 * i + sub;
-        const int f = __shfl_sync(0xffffffffu, myidx, kk);
+        const int f = __shfl_sync(0xffffffffu, idx_cur, kk);
         const int k = pw * RPW + kk;
         // row k of the image, chunk (c&7) XOR (k&7): the 128-byte swizzle of the UMMA / TMA layouts
         const uint32_t dst = (dst0 + k * 128) ^ ((uint32_t)(k & 7) << 4);
@@ -220,14 +235,14 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     if (lane == 0) {
       constexpr uint32_t idesc = make_idesc_bf16(128, G, /*A MN-major*/ 1, /*B K-major*/ 0);
       for (int T = 0; T < total; ++T) {
-        const int gl = T / ntp, which = T - gl * ntp;
-        const int ws = gl & 1, hs = T % C::HS, slot = T % C::NSLOT;
-        if (which == 0) mbar_wait(&w_full[ws], (gl >> 1) & 1);
+        const int gl = T >> tsh, which = T & tsh;
+        const int ws = gl % C::WS, hs = T % C::HS, slot = T % C::NSLOT;
+        if (which == 0) mbar_wait(&w_full[ws], (gl / C::WS) & 1);
         mbar_wait(&h_full[hs], (T / C::HS) & 1);
         mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
         tc_fence_after();
-        const uint32_t a0 = smem_u32(smem + C::OFF_H + hs * C::H_BYTES);
-        const uint32_t b0 = smem_u32(smem + C::OFF_W + ws * C::W_BYTES);
+        const uint32_t a0 = sbase + C::OFF_H + hs * C::H_BYTES;
+        const uint32_t b0 = sbase + C::OFF_W + ws * C::W_BYTES;
         const uint32_t d = tmem_base + slot * G;
 #pragma unroll
         for (int j = 0; j < K / 16; ++j) {
@@ -237,16 +252,16 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         }
         umma_commit(&h_empty[hs]);
         umma_commit(&t_full[slot]);
-        if (which == ntp - 1) umma_commit(&w_empty[ws]);
+        if (which == tsh) umma_commit(&w_empty[ws]);
       }
     }
   } else if (warp == 13) {
     // ===================== W loader =====================
     if (lane == 0) {
       for (int gl = 0; gl < ngl; ++gl) {
-        const int ws = gl & 1;
+        const int ws = gl % C::WS;
         const int64_t g = stripe + (int64_t)gl * p.S;
-        mbar_wait(&w_empty[ws], ((gl >> 1) & 1) ^ 1);
+        mbar_wait(&w_empty[ws], ((gl / C::WS) & 1) ^ 1);
         mbar_arrive_expect_tx(&w_full[ws], C::W_BYTES);
 #pragma unroll
         for (int kb = 0; kb < K / 64; ++kb)
@@ -254,9 +269,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
       }
     }
   } else {
-    // ===================== epilogue =====================
+    // ===================== epilogue: every warp is self-contained (own rows, own staging, own TMA stores) =====
     const int half = warp >> 2, q = warp & 3;
-    const int tih = threadIdx.x & 127;                         // thread index inside the half
     const int row = q * 32 + lane;                             // row of the batch tile == TMEM lane
     const int my_bt = 2 * pr + (ntp == 2 ? half : 0);
     const int b = my_bt * 128 + row;
@@ -269,17 +283,26 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     }
     float loss_local = 0.f;
     const float hs = 0.5f * p.s;
-    uint8_t* stage = smem + C::OFF_ST + half * C::ST_BYTES;
-    float* sbias = reinterpret_cast<float*>(smem + C::OFF_BIAS) + half * G;
-    const bool issuer = tih == 0;
+    // this warp's 32 rows of the half's staging tile(s); rows are 128 B (G >= 64) or 64 B (G = 32)
+    constexpr int ROWB = G >= 64 ? 128 : 64;
+    const uint32_t stage_w = sbase + C::OFF_ST + half * C::ST_BYTES + q * 32 * ROWB;
+    const uint32_t stage_row = stage_w + lane * ROWB;
+    const uint32_t swz = G >= 64 ? (uint32_t)(lane & 7) : (uint32_t)((lane >> 1) & 3);
+    const uint32_t sbias_w = sbase + C::OFF_BIAS + warp * G * 4;
     for (int T = half; T < total; T += 2) {
-      const int gl = T / ntp;
+      const int gl = T >> tsh;
       const int64_t g = stripe + (int64_t)gl * p.S;
       const int nl = (int)min((int64_t)G, p.L - g * G);
       const int slot = T % C::NSLOT;
-      if (issuer) bulk_wait_read<0>();                         // the staging tile is free again
-      if (p.bias && tih < G) sbias[tih] = tih < nl ? __ldg(p.bias + g * G + tih) : 0.f;
-      named_bar_sync(1 + half, 128);
+      if (lane == 0) bulk_wait_read<0>();                      // this warp's previous TMA store has read the staging rows
+      if (p.bias) {
+#pragma unroll
+        for (int i = 0; i < G / 32; ++i) {
+          const int l = i * 32 + lane;
+          sts32(sbias_w + l * 4, __float_as_uint(l < nl ? __ldg(p.bias + g * G + l) : 0.f));
+        }
+      }
+      __syncwarp();
       // positives of this row inside the group: walk the CSR cursor (ascending groups, fixed row)
       const int64_t glo64 = p.label_offset + g * G;
       const int glo = (int)min(glo64, (int64_t)0x7fffffff), ghi = (int)min(glo64 + nl, (int64_t)0x7fffffff);
@@ -319,12 +342,13 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         uint32_t out[16];
         float* zout = (p.logits && valid_row) ? p.logits + (size_t)b * p.L + g * G + sc * 32 : nullptr;
         const int nvalid = nl - sc * 32;
+        const uint32_t sb = sbias_w + sc * 128;
         if (slow) {
-          if (p.bias) epi32<true, true>(v[sc & 1], sbias + sc * 32, ym[sc], nvalid, p.s, hs, R, P, out, zout);
-          else epi32<true, false>(v[sc & 1], nullptr, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+          if (p.bias) epi32<true, true>(v[sc & 1], sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+          else epi32<true, false>(v[sc & 1], sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
         } else {
-          if (p.bias) epi32<false, true>(v[sc & 1], sbias + sc * 32, 0u, 32, p.s, hs, R, P, out, nullptr);
-          else epi32<false, false>(v[sc & 1], nullptr, 0u, 32, p.s, hs, R, P, out, nullptr);
+          if (p.bias) epi32<false, true>(v[sc & 1], sb, 0u, 32, p.s, hs, R, P, out, nullptr);
+          else epi32<false, false>(v[sc & 1], sb, 0u, 32, p.s, hs, R, P, out, nullptr);
         }
         if (sc & 1) {   // 64 factors in [1/2,1) at most per product: fold into the loss, restart the chains
           loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
@@ -332,36 +356,29 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
           for (int i = 0; i < 4; ++i) { R[i] = 0.f; P[i] = 1.f; }
         }
         if (p.write_dy) {
-          if (G >= 64) {
-            uint8_t* rowp = stage + (sc >> 1) * 16384 + row * 128;
+          if (G > 64 && sc == 2) {        // second 64-label half of a wide group reuses the staging rows
+            if (lane == 0) bulk_wait_read<0>();
+            __syncwarp();
+          }
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const int ch = ((sc & 1) * 4 + i) ^ (row & 7);
-              *reinterpret_cast<uint4*>(rowp + ch * 16) = make_uint4(out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
-            }
-          } else {
-            uint8_t* rowp = stage + row * 64;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const int ch = i ^ ((row >> 1) & 3);
-              *reinterpret_cast<uint4*>(rowp + ch * 16) = make_uint4(out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
+          for (int i = 0; i < 4; ++i) {
+            const uint32_t ch = (uint32_t)((G >= 64 ? (sc & 1) * 4 : 0) + i) ^ swz;
+            sts128(stage_row + ch * 16, out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
+          }
+          if (sc == G / 32 - 1 || (G > 64 && sc == 1)) {
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_3d(&tmY, smem + C::OFF_ST + half * C::ST_BYTES + q * 32 * ROWB, (sc >> 1) * 64, my_bt * 128 + q * 32, (int)g);
+              bulk_commit();
             }
           }
         }
       }
       if ((G / 32) & 1)
         loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
-      if (p.write_dy) fence_proxy_async_smem();
-      named_bar_sync(1 + half, 128);
-      if (p.write_dy) {
-        if (issuer) {
-#pragma unroll
-          for (int sb = 0; sb < (G + 63) / 64; ++sb) tma_store_3d(&tmY, stage + sb * 16384, sb * 64, my_bt * 128, (int)g);
-          bulk_commit();
-        }
-      }
     }
-    if (issuer) bulk_wait<0>();
+    if (lane == 0) bulk_wait<0>();
     if (!valid_row) loss_local = 0.f;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) loss_local += __shfl_xor_sync(0xffffffffu, loss_local, o);
@@ -428,7 +445,7 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   if (dY) {
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
     const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
-    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 128, 1};
+    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 32, 1};   // one epilogue warp's 32 rows
     int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
     if (rc) return rc;
   } else {
