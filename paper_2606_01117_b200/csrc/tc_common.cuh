@@ -13,6 +13,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "../../include/haste.h"
+
 namespace haste {
 namespace tc {
 
@@ -183,8 +185,16 @@ __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, int a_mn_ma
 }  // namespace tc
 
 // ---------------------------------------------------------------- host: tensor maps
-// bf16 tensor of `rank` dims (dim 0 innermost), 128-byte swizzle, box given in elements.
-int encode_tmap_bf16(CUtensorMap* out, const void* base, int rank, const uint64_t* dims, const uint64_t* strides_bytes,
-                     const uint32_t* box);
+// Tensor of `rank` dims (dim 0 innermost), element size dtype_bytes (2 = bf16, 4 = fp32), box in elements,
+// swizzle_bytes in {0, 32, 64, 128}.  Out-of-bounds box elements are zero-filled on load, dropped on store.
+int encode_tmap(CUtensorMap* out, int dtype_bytes, const void* base, int rank, const uint64_t* dims,
+                const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
+
+// State of one sparse-tail handle's tcgen05 family (tc_tail.cu owns create / destroy).
+struct TcTailState {
+  haste_config_t cfg;
+  int device, num_sms, Bpad;
+  int n_partials;
+};
 
 }  // namespace haste

@@ -1,0 +1,294 @@
+// tc_dw.cu -- tcgen05 weight-gradient kernel of the HASTE sparse tail (sm_100a; bf16 in, fp32 accumulate).
+//
+//   dW_g [G x K] = dY_g^T [G x B] * H_g [B x K],  H_g = X[:, idx_g]
+//   db_g [G]     = dY_g^T * 1
+//
+// Persistent CTAs, one per SM, groups strided over the grid.  The batch (the contraction) is streamed in
+// k-blocks of 64 rows through a shared-memory ring:
+//   A operand (M = labels): the dY k-block [64 batch rows][G labels] exactly as it sits in HBM (one TMA box per
+//     64 labels, 128-byte swizzle) read as an MN-major operand -- no transposition anywhere;
+//   B operand (N = fan-in slots): H^T k-block [K rows][64 batch] gathered from X^T with 16-byte cp.async
+//     (a row of X^T is one feature, batch contiguous), K-major; the image carries a few extra rows of
+//     ones, so accumulator column K is sum_b dY[b][l] = db[l] at no extra operand traffic.
+//   D [G lanes x (K + extra) columns] fp32 in TMEM, double buffered across groups.
+// warp roles (320 threads): warps 0-3 epilogue (TMEM -> registers -> swizzled smem rows -> TMA store of dW
+// rows; a thread owns one label, so a dW row is written as it is stored), warps 4-7 gather producers,
+// warp 8 MMA issuer, warp 9 TMA loader of dY.
+#include <algorithm>
+
+#include "tc_common.cuh"
+#include "tc_kernels.h"
+
+namespace haste {
+using namespace tc;
+
+struct DwParams {
+  const bf16* Xt;       // [d][Bpad], zero for b >= B up to the next multiple of 128
+  const int32_t* idx;   // [NG][K]
+  float* dbias;         // [L] or null
+  int write_dw;
+  int B, Bpad, NKB;     // NKB = ceil(B / 64) k-blocks
+  int64_t L, NG;
+};
+
+template <int G, int K, bool F32> struct DwCfg {
+  static constexpr int NE = G == 128 ? 16 : 8;              // rows of ones appended to the H image
+  static constexpr int N = K + NE;                          // MMA N
+  static constexpr int H_BYTES = (K + 16) * 128;            // multiple of 1024
+  static constexpr int Y_BYTES = G * 128;                   // [G/64 atoms][64 rows][128 B]
+  static constexpr int STAGE = H_BYTES + Y_BYTES;
+  static constexpr int EPI_BYTES = 4 * 2 * 4096;            // 4 warps x 2 buffers x [32 rows][128 B]
+  static constexpr int NST_RAW = (232448 - 1024 - EPI_BYTES - 1024) / STAGE;
+  static constexpr int NST = NST_RAW > 8 ? 8 : NST_RAW;
+  static constexpr int LAG = 2;
+  static constexpr int TS = N <= 128 ? 128 : 256;           // TMEM columns per accumulator slot
+  static constexpr int OFF_EPI = NST * STAGE;
+  static constexpr int OFF_BAR = OFF_EPI + EPI_BYTES;
+  static constexpr int NBAR = 2 * NST + 4;
+  static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;
+  static constexpr int SMEM = OFF_MISC + 64 + 1024;
+  static constexpr int RW = G == 128 ? 32 : 16;             // label rows per epilogue warp (M = 64 fills lanes 0-15 of a quadrant)
+  static constexpr int NBOX = F32 ? K / 32 : K / 64;        // 128-byte output boxes per dW row
+  static_assert(NST > LAG, "ring too short");
+};
+
+__device__ __forceinline__ uint32_t dw_pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ uint32_t tmem_ld1(uint32_t taddr) {
+  uint32_t v;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(taddr) : "memory");
+  return v;
+}
+
+template <int G, int K, bool F32>
+__global__ void __launch_bounds__(320, 1)
+tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmO, const DwParams p) {
+  using C = DwCfg<G, K, F32>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t sbase = smem_u32(smem);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
+  uint64_t* full = bars;                    // [NST] count 5: 4 producer warps + the TMA thread (expect_tx)
+  uint64_t* empty = bars + C::NST;          // [NST] count 1: umma commit
+  uint64_t* t_full = bars + 2 * C::NST;     // [2]   count 1: umma commit
+  uint64_t* t_empty = t_full + 2;           // [2]   count 4: epilogue warps
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_my = p.NG > blockIdx.x ? (int)((p.NG - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;   // groups of this CTA
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], 5); mbar_init(&empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
+    fence_barrier_init();
+  }
+  // rows K .. K+15 of every stage's H image: bf16 1.0 (swizzling permutes equal chunks: write linearly)
+  for (int e = threadIdx.x; e < C::NST * 16 * 8; e += blockDim.x) {
+    const int st = e / 128, r = e % 128;
+    sts128(sbase + st * C::STAGE + K * 128 + r * 16, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
+  }
+  fence_proxy_async_smem();
+  if (warp == 9 && lane == 0) { tma_prefetch_desc(&tmY); tma_prefetch_desc(&tmO); }
+  if (warp == 8) tmem_alloc<2 * C::TS>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp >= 4 && warp < 8) {
+    // ===================== gather producers =====================
+    const int pw = warp - 4;
+    constexpr int RPW = K / 4;                       // slots per producer warp
+    const int sub = lane >> 3, c = lane & 7;         // 4 rows per instruction, 8 chunks of 16 B per row
+    const int32_t* idx_ptr = p.idx + pw * RPW + lane;
+    int idx_cur = 0, idx_nxt = 0;
+    if (lane < RPW && n_my > 0) idx_nxt = __ldg(idx_ptr + (int64_t)blockIdx.x * K);
+    int it = 0;
+    for (int i = 0; i < n_my; ++i) {
+      const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+      idx_cur = idx_nxt;
+      if (lane < RPW && i + 1 < n_my) idx_nxt = __ldg(idx_ptr + (g + gridDim.x) * K);
+      for (int kb = 0; kb < p.NKB; ++kb, ++it) {
+        const int st = it % C::NST;
+        mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
+        const uint32_t dst0 = sbase + st * C::STAGE;
+        const bf16* src0 = p.Xt + kb * 64 + c * 8;
+#pragma unroll
+        for (int r4 = 0; r4 < RPW / 4; ++r4) {
+          const int rr = 4 * r4 + sub;
+          const int f = __shfl_sync(0xffffffffu, idx_cur, rr);
+          const int row = pw * RPW + rr;
+          cp_async16(dst0 + row * 128 + (((uint32_t)(c ^ (row & 7))) << 4), src0 + (size_t)f * p.Bpad);
+        }
+        cp_async_commit();
+        if (it >= C::LAG) {
+          cp_async_wait<C::LAG>();
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&full[(it - C::LAG) % C::NST]);
+        }
+      }
+    }
+#pragma unroll
+    for (int r = C::LAG - 1; r >= 0; --r) {
+      const int T = it - 1 - r;
+      if (T >= 0) {
+        if (r == 1) cp_async_wait<1>(); else cp_async_wait<0>();
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[T % C::NST]);
+      }
+    }
+  } else if (warp == 8) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = make_idesc_bf16(G, C::N, /*A (dY) MN-major*/ 1, /*B (H^T) K-major*/ 0);
+      int it = 0;
+      for (int i = 0; i < n_my; ++i) {
+        const int slot = i & 1;
+        mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t d = tmem_base + slot * C::TS;
+        for (int kb = 0; kb < p.NKB; ++kb, ++it) {
+          const int st = it % C::NST;
+          mbar_wait(&full[st], (it / C::NST) & 1);
+          tc_fence_after();
+          const uint32_t h0 = sbase + st * C::STAGE, y0 = h0 + C::H_BYTES;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const uint64_t ad = make_sdesc_sw128(y0 + j * 2048, 8192, 1024);
+            const uint64_t bd = make_sdesc_sw128(h0 + j * 32, 16, 1024);
+            umma_f16(d, ad, bd, idesc, (kb | j) ? 1u : 0u);
+          }
+          umma_commit(&empty[st]);
+        }
+        umma_commit(&t_full[slot]);
+      }
+    }
+  } else if (warp == 9) {
+    // ===================== TMA loader of dY k-blocks =====================
+    if (lane == 0) {
+      int it = 0;
+      for (int i = 0; i < n_my; ++i) {
+        const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+        for (int kb = 0; kb < p.NKB; ++kb, ++it) {
+          const int st = it % C::NST;
+          mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
+          mbar_arrive_expect_tx(&full[st], C::Y_BYTES);
+#pragma unroll
+          for (int a = 0; a < G / 64; ++a)
+            tma_load_3d(smem + st * C::STAGE + C::H_BYTES + a * 8192, &tmY, &full[st], a * 64, kb * 64, (int)g);
+        }
+      }
+    }
+  } else {
+    // ===================== epilogue =====================
+    const int q = warp;                                         // TMEM lane quadrant
+    const uint32_t sbuf0 = sbase + C::OFF_EPI + q * 8192;
+    const uint32_t swz = (uint32_t)(lane & 7);
+    int nstore = 0;
+    for (int i = 0; i < n_my; ++i) {
+      const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+      const int slot = i & 1;
+      mbar_wait(&t_full[slot], (i >> 1) & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * C::TS;
+      if (p.write_dw) {
+#pragma unroll 1
+        for (int c = 0; c < C::NBOX; ++c, ++nstore) {
+          uint32_t out[32];
+          if (F32) {
+            tmem_ld32(taddr + c * 32, out);
+            tmem_ld_wait();
+          } else {
+            uint32_t v0[32], v1[32];
+            tmem_ld32(taddr + c * 64, v0);
+            tmem_ld32(taddr + c * 64 + 32, v1);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              out[j] = dw_pack_bf16x2(__uint_as_float(v0[2 * j]), __uint_as_float(v0[2 * j + 1]));
+              out[16 + j] = dw_pack_bf16x2(__uint_as_float(v1[2 * j]), __uint_as_float(v1[2 * j + 1]));
+            }
+          }
+          const uint32_t sbuf = sbuf0 + (nstore & 1) * 4096;
+          if (lane == 0) bulk_wait_read<1>();                   // the store issued from this buffer two boxes ago has read it
+          __syncwarp();
+#pragma unroll
+          for (int ch = 0; ch < 8; ++ch)
+            sts128(sbuf + lane * 128 + ((ch ^ swz) << 4), out[4 * ch], out[4 * ch + 1], out[4 * ch + 2], out[4 * ch + 3]);
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 8192 + (nstore & 1) * 4096, c * (F32 ? 32 : 64), (int)(g * G + q * C::RW));
+            bulk_commit();
+          }
+        }
+      }
+      if (p.dbias) {
+        const uint32_t v = tmem_ld1(taddr + K);
+        tmem_ld_wait();
+        const int64_t l = g * G + q * C::RW + lane;
+        if (lane < C::RW && l < p.L) p.dbias[l] = __uint_as_float(v);
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&t_empty[slot]);
+    }
+    if (lane == 0) bulk_wait<0>();
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 8) { tc_fence_after(); tmem_dealloc<2 * C::TS>(tmem_base); }
+}
+
+template <int G, int K, bool F32>
+static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
+                     float* dbias, cudaStream_t st) {
+  using C = DwCfg<G, K, F32>;
+  static_assert(C::SMEM <= 232448, "shared memory budget");
+  CUtensorMap tmY, tmO;
+  {
+    const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
+    const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
+    const uint32_t box[3] = {64, 64, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, 128);
+    if (rc) return rc;
+  }
+  if (dW) {
+    const int es = F32 ? 4 : 2;
+    const uint64_t dims[2] = {(uint64_t)K, (uint64_t)sh.L};
+    const uint64_t str[1] = {(uint64_t)K * es};
+    const uint32_t box[2] = {(uint32_t)(128 / es), (uint32_t)C::RW};
+    int rc = encode_tmap(&tmO, es, dW, 2, dims, str, box, 128);
+    if (rc) return rc;
+  } else {
+    tmO = tmY;
+  }
+  DwParams p;
+  p.Xt = (const bf16*)Xt; p.idx = idx; p.dbias = dbias; p.write_dw = dW ? 1 : 0;
+  p.B = sh.B; p.Bpad = sh.Bpad; p.NKB = ceil_div(sh.B, 64); p.L = sh.L; p.NG = sh.NG;
+  const int grid = (int)std::min<int64_t>(sh.NG, s->num_sms);
+  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dw_kernel<G, K, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+  tc_dw_kernel<G, K, F32><<<grid, 320, C::SMEM, st>>>(tmY, tmO, p);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
+               float* dbias, cudaStream_t st, int* n_launches) {
+  *n_launches = 1;
+  const bool f32 = s->cfg.dw_dtype == HASTE_F32;
+#define HASTE_DW(G_, K_)                                                                     \
+  if (sh.G == G_ && sh.K == K_)                                                              \
+    return f32 ? launch_dw<G_, K_, true>(s, sh, Xt, idx, dY, dW, dbias, st)                  \
+               : launch_dw<G_, K_, false>(s, sh, Xt, idx, dY, dW, dbias, st)
+  HASTE_DW(64, 128); HASTE_DW(64, 64); HASTE_DW(128, 64); HASTE_DW(128, 128);
+#undef HASTE_DW
+  return HASTE_ERR_UNSUPPORTED;   // G = 32: the caller runs the CUDA-core kernel
+}
+
+}  // namespace haste

@@ -399,12 +399,6 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-struct TcTailState {
-  haste_config_t cfg;
-  int device, num_sms, Bpad;
-  int n_partials;
-};
-
 bool tc_tail_supported(const haste_config_t& cfg, int) {
   if (cfg.dtype != HASTE_BF16) return false;
   if (!(cfg.G == 32 || cfg.G == 64 || cfg.G == 128)) return false;
@@ -476,13 +470,6 @@ int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const i
   HASTE_FWD(64, 128); HASTE_FWD(64, 64); HASTE_FWD(32, 64); HASTE_FWD(32, 128); HASTE_FWD(128, 64); HASTE_FWD(128, 128);
 #undef HASTE_FWD
   set_error("tcgen05 forward: unsupported (G, K)");
-  return HASTE_ERR_UNSUPPORTED;
-}
-
-int tc_tail_dw(TcTailState*, const TailShape&, const void*, const int32_t*, const void*, void*, float*, cudaStream_t, int*) {
-  return HASTE_ERR_UNSUPPORTED;
-}
-int tc_tail_dx(TcTailState*, const TailShape&, const int32_t*, const void*, const void*, float*, cudaStream_t, int*) {
   return HASTE_ERR_UNSUPPORTED;
 }
 
