@@ -27,17 +27,22 @@ struct DwParams {
   const int32_t* idx;   // [NG][K]
   float* dbias;         // [L] or null
   int write_dw;
-  int B, Bpad, NKB;     // NKB = ceil(B / 64) k-blocks
+  int B, Bpad, NKB;     // NKB = ceil(B / 128) k-blocks
   int64_t L, NG;
 };
 
 template <int G, int K, bool F32> struct DwCfg {
   static constexpr int NE = G == 128 ? 16 : 8;              // rows of ones appended to the H image
   static constexpr int N = K + NE;                          // MMA N
-  static constexpr int H_BYTES = (K + 16) * 128;            // multiple of 1024
-  static constexpr int Y_BYTES = G * 128;                   // [G/64 atoms][64 rows][128 B]
+  // a k-block is 128 batch rows = two 64-row halves (one 128-byte swizzle row holds 64 bf16): the issuing thread
+  // pays one barrier wait and one commit per 8 MMAs (with 64-row k-blocks its ~0.3 us loop overhead per k-block
+  // was the kernel's bottleneck)
+  static constexpr int HH_BYTES = (K + 16) * 128;           // one half of the H image, multiple of 1024
+  static constexpr int YH_BYTES = G * 128;                  // one half of the dY image: [G/64 atoms][64 rows][128 B]
+  static constexpr int H_BYTES = 2 * HH_BYTES;
+  static constexpr int Y_BYTES = 2 * YH_BYTES;
   static constexpr int STAGE = H_BYTES + Y_BYTES;
-  static constexpr int EPI_BYTES = 4 * 2 * 4096;            // 4 warps x 2 buffers x [32 rows][128 B]
+  static constexpr int EPI_BYTES = 4 * 4096;                // 4 warps x [32 rows][128 B]
   static constexpr int NST_RAW = (232448 - 1024 - EPI_BYTES - 1024) / STAGE;
   static constexpr int NST = NST_RAW > 8 ? 8 : NST_RAW;
   static constexpr int LAG = 2;
@@ -85,9 +90,9 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     fence_barrier_init();
   }
   // rows K .. K+15 of every stage's H image: bf16 1.0 (swizzling permutes equal chunks: write linearly)
-  for (int e = threadIdx.x; e < C::NST * 16 * 8; e += blockDim.x) {
-    const int st = e / 128, r = e % 128;
-    sts128(sbase + st * C::STAGE + K * 128 + r * 16, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
+  for (int e = threadIdx.x; e < C::NST * 2 * 16 * 8; e += blockDim.x) {
+    const int st = e / 256, hf = (e >> 7) & 1, r = e % 128;
+    sts128(sbase + st * C::STAGE + hf * C::HH_BYTES + K * 128 + r * 16, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
   }
   fence_proxy_async_smem();
   if (warp == 9 && lane == 0) { tma_prefetch_desc(&tmY); tma_prefetch_desc(&tmO); }
@@ -114,13 +119,16 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
         const int st = it % C::NST;
         mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
         const uint32_t dst0 = sbase + st * C::STAGE;
-        const bf16* src0 = p.Xt + kb * 64 + c * 8;
+        const bf16* src0 = p.Xt + kb * 128 + c * 8;
 #pragma unroll
         for (int r4 = 0; r4 < RPW / 4; ++r4) {
           const int rr = 4 * r4 + sub;
           const int f = __shfl_sync(0xffffffffu, idx_cur, rr);
           const int row = pw * RPW + rr;
-          cp_async16(dst0 + row * 128 + (((uint32_t)(c ^ (row & 7))) << 4), src0 + (size_t)f * p.Bpad);
+          const uint32_t dst = dst0 + row * 128 + (((uint32_t)(c ^ (row & 7))) << 4);
+          const bf16* src = src0 + (size_t)f * p.Bpad;
+          cp_async16(dst, src);
+          cp_async16(dst + C::HH_BYTES, src + 64);
         }
         cp_async_commit();
         if (it >= C::LAG) {
@@ -157,9 +165,9 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           tc_fence_after();
           const uint32_t h0 = sbase + st * C::STAGE, y0 = h0 + C::H_BYTES;
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const uint64_t ad = make_sdesc_sw128(y0 + j * 2048, 8192, 1024);
-            const uint64_t bd = make_sdesc_sw128(h0 + j * 32, 16, 1024);
+          for (int j = 0; j < 8; ++j) {
+            const uint64_t ad = make_sdesc_sw128(y0 + (j >> 2) * C::YH_BYTES + (j & 3) * 2048, 8192, 1024);
+            const uint64_t bd = make_sdesc_sw128(h0 + (j >> 2) * C::HH_BYTES + (j & 3) * 32, 16, 1024);
             umma_f16(d, ad, bd, idesc, (kb | j) ? 1u : 0u);
           }
           umma_commit(&empty[st]);
@@ -178,15 +186,18 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
           mbar_arrive_expect_tx(&full[st], C::Y_BYTES);
 #pragma unroll
-          for (int a = 0; a < G / 64; ++a)
-            tma_load_3d(smem + st * C::STAGE + C::H_BYTES + a * 8192, &tmY, &full[st], a * 64, kb * 64, (int)g);
+          for (int hf = 0; hf < 2; ++hf)
+#pragma unroll
+            for (int a = 0; a < G / 64; ++a)
+              tma_load_3d(smem + st * C::STAGE + C::H_BYTES + hf * C::YH_BYTES + a * 8192, &tmY, &full[st], a * 64,
+                          kb * 128 + hf * 64, (int)g);
         }
       }
     }
   } else {
     // ===================== epilogue =====================
     const int q = warp;                                         // TMEM lane quadrant
-    const uint32_t sbuf0 = sbase + C::OFF_EPI + q * 8192;
+    const uint32_t sbuf0 = sbase + C::OFF_EPI + q * 4096;
     const uint32_t swz = (uint32_t)(lane & 7);
     int nstore = 0;
     for (int i = 0; i < n_my; ++i) {
@@ -213,8 +224,8 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
               out[16 + j] = dw_pack_bf16x2(__uint_as_float(v1[2 * j]), __uint_as_float(v1[2 * j + 1]));
             }
           }
-          const uint32_t sbuf = sbuf0 + (nstore & 1) * 4096;
-          if (lane == 0) bulk_wait_read<1>();                   // the store issued from this buffer two boxes ago has read it
+          const uint32_t sbuf = sbuf0;
+          if (lane == 0) bulk_wait_read<0>();                   // the previous store has read the staging rows
           __syncwarp();
 #pragma unroll
           for (int ch = 0; ch < 8; ++ch)
@@ -222,7 +233,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 8192 + (nstore & 1) * 4096, c * (F32 ? 32 : 64), (int)(g * G + q * C::RW));
+            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 4096, c * (F32 ? 32 : 64), (int)(g * G + q * C::RW));
             bulk_commit();
           }
         }
@@ -270,7 +281,7 @@ static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const 
   }
   DwParams p;
   p.Xt = (const bf16*)Xt; p.idx = idx; p.dbias = dbias; p.write_dw = dW ? 1 : 0;
-  p.B = sh.B; p.Bpad = sh.Bpad; p.NKB = ceil_div(sh.B, 64); p.L = sh.L; p.NG = sh.NG;
+  p.B = sh.B; p.Bpad = sh.Bpad; p.NKB = ceil_div(sh.B, 128); p.L = sh.L; p.NG = sh.NG;
   const int grid = (int)std::min<int64_t>(sh.NG, s->num_sms);
   HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dw_kernel<G, K, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
   tc_dw_kernel<G, K, F32><<<grid, 320, C::SMEM, st>>>(tmY, tmO, p);
