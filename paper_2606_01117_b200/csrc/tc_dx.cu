@@ -9,6 +9,8 @@
 //   feature row).  The reduction over groups happens in L2: 1.47 T adds/s measured
 //   (profiles/r01_probe_microbench.txt), which bounds this version.
 #include <algorithm>
+#include <cstdlib>
+#include <cstring>
 
 #include "tc_common.cuh"
 #include "tc_kernels.h"
@@ -147,6 +149,7 @@ tc_dx_red_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
   if (warp == 4) { tc_fence_after(); tmem_dealloc<2 * K>(tmem_base); }
 }
 
+
 template <int G, int K>
 static int launch_dx_red(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                          cudaStream_t st) {
@@ -180,7 +183,10 @@ static int launch_dx_red(TcTailState* s, const TailShape& sh, const int32_t* idx
 int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                cudaStream_t st, int* n_launches) {
   *n_launches = 1;
-#define HASTE_DX(G_, K_) if (sh.G == G_ && sh.K == K_) return launch_dx_red<G_, K_>(s, sh, idx, W, dY, dXt, st)
+  static const bool use_red = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "red");   // first version, for comparison
+#define HASTE_DX(G_, K_)                                                                   \
+  if (sh.G == G_ && sh.K == K_)                                                            \
+    return use_red ? launch_dx_red<G_, K_>(s, sh, idx, W, dY, dXt, st) : tc_tail_dx_acc(s, sh, idx, W, dY, dXt, st)
   HASTE_DX(64, 128); HASTE_DX(64, 64); HASTE_DX(128, 64); HASTE_DX(128, 128);
 #undef HASTE_DX
   return HASTE_ERR_UNSUPPORTED;   // G = 32: the caller runs the CUDA-core kernel

@@ -1,0 +1,384 @@
+// tc_dx_acc.cu -- input-gradient kernel of the HASTE sparse tail with the reduction over groups kept ON CHIP
+// (sm_100a; bf16 in, fp32 accumulate).
+//
+//   dX[:, idx_g] += dY_g [B x G] * W_g [G x K]   over all groups g
+//
+// Why: the B*NG*K scatter-adds (669 M at config 3) go through L2 reductions at no more than ~1.47 T adds/s
+// (profiles/r01_probe_microbench.txt), 3.5x the kernel's HBM floor, and a shared-memory accumulator for all d
+// features of a 128-row batch tile does not fit (d * 512 B).  Measured on this B200
+// (profiles/r01_probe_onchip_rmw.txt): read-modify-write of a thread-owned word runs at ~12 adds/clk/SM in
+// shared memory AND at ~12 adds/clk/SM in tensor memory (tcgen05.ld/st .x1 at a dynamic column); the two, and
+// the L2 reduction path, are independent resources.  So the features are split by id into five classes, and
+// because an idx row is sorted each class is a contiguous slot range of every group:
+//     TA = [0, fa)   TC = [fa, f1)   fp32 accumulator COLUMNS in TMEM (next to the two P buffers)
+//     SB = [f1, fb)  SD = [fb, f2)   fp32 accumulator ROWS in shared memory ([f2-f1][128 batch] floats)
+//     L  = [f2, d)                   red.global.add.f32 into dX^T, as in the first version (tc_dx.cu)
+// A CTA owns (128-row batch tile, stripe of groups).  Per group: TMA loads the dY tile and W_g, one thread
+// issues P^T[128 batch x K slots] = dY tile * W_g (tcgen05, fp32 in TMEM, double buffered), an auxiliary
+// warp turns idx_g into one destination list per class, and 16 epilogue warps (4 sets x 4 TMEM lane
+// quadrants; a lane owns one batch row) add column j of P into the destination of slot j.  Set s owns class s
+// exclusively, so no two threads ever touch the same accumulator word and nothing on chip is atomic; the L
+// chunks are dealt round-robin to the four sets (they are atomic in L2).  Lists are padded to whole chunks with
+// a dummy destination per class (a spare TMEM column, a spare shared-memory row), so the on-chip
+// inner loops carry no predicates; only the last L chunk is predicated (a dummy word in L2 would be one address
+// hammered by every CTA).  Groups whose idx row is not strictly increasing (duplicates, unsorted:
+// legal by DESIGN.md reading R4) take the L path for every slot, which is correct for any index row.
+// The accumulators are flushed into dX^T once per CTA.
+#include <algorithm>
+#include <cstdlib>
+
+#include "tc_common.cuh"
+#include "tc_kernels.h"
+
+namespace haste {
+using namespace tc;
+
+struct DxAccParams {
+  float* dXt;           // [d][Bpad] fp32, zeroed by the caller
+  const int32_t* idx;   // [NG][K]
+  int B, Bpad, NT, S, d;
+  int64_t NG;
+  int fa, f1, fb, f2;   // class boundaries (see above)
+};
+
+template <int G, int K> struct DxAccCfg {
+  static constexpr int NSET = 4;                              // epilogue sets: 0 = TA, 1 = SB, 2 = TC, 3 = SD
+  static constexpr int NLIST = NSET + 1;                      // + the L list
+  static constexpr int Y_BYTES = G * 256;                     // [G/64 k-blocks][128 batch rows][128 B]
+  static constexpr int W_BYTES = G * K * 2;                   // [K/64 slot atoms][G label rows][128 B]
+  static constexpr int STAGE = Y_BYTES + W_BYTES;
+  static constexpr int NST = STAGE <= 32768 ? 3 : 2;
+  static constexpr int LIST_LEN = K + 16;                     // entries per list (padding for the last chunk)
+  static constexpr int RING_META = 64;                        // lo[5], n[5]
+  static constexpr int RING_BYTES = (RING_META + K * 4 + NLIST * LIST_LEN * 4 + 127) / 128 * 128;
+  static constexpr int RD = 4;                                // depth of the destination-list ring
+  static constexpr int TF = 512 - 2 * K - 16;                 // TMEM accumulator columns usable by features
+  static constexpr int TDUMMY = 2 * K + TF;                   // dummy TMEM column (first of the 16 spare ones)
+  static constexpr int OFF_RING = NST * STAGE;
+  static constexpr int OFF_BAR = OFF_RING + RD * RING_BYTES;
+  static constexpr int NBAR = 2 * NST + 4 + 2 * RD;
+  static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;
+  static constexpr int OFF_ACC = (OFF_MISC + 64 + 511) / 512 * 512;
+  static constexpr int NS_MAX = (232448 - 1024 - OFF_ACC) / 512 - 1;   // shared-memory accumulator rows (+1 dummy row)
+  static_assert(NS_MAX >= 16, "no room for shared-memory accumulators");
+  static constexpr int THREADS = (4 * NSET + 3) * 32;
+};
+
+__device__ __forceinline__ void dxa_red_add_f32(float* addr, float v) {
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t dxa_tld1(uint32_t taddr) {
+  uint32_t v;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(taddr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void dxa_tst1(uint32_t taddr, uint32_t v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void dxa_tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ int4 dxa_lds128i(uint32_t addr) {
+  int4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ int dxa_lds32i(uint32_t addr) {
+  int v;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ float dxa_lds32f(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void dxa_sts32f(uint32_t addr, float v) {
+  asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+// 16 destination codes of one chunk of a list
+__device__ __forceinline__ void dxa_load_dest(uint32_t addr, int (&dst)[16]) {
+  const int4 a0 = dxa_lds128i(addr), a1 = dxa_lds128i(addr + 16), a2 = dxa_lds128i(addr + 32), a3 = dxa_lds128i(addr + 48);
+  dst[0] = a0.x; dst[1] = a0.y; dst[2] = a0.z; dst[3] = a0.w; dst[4] = a1.x; dst[5] = a1.y; dst[6] = a1.z; dst[7] = a1.w;
+  dst[8] = a2.x; dst[9] = a2.y; dst[10] = a2.z; dst[11] = a2.w; dst[12] = a3.x; dst[13] = a3.y; dst[14] = a3.z; dst[15] = a3.w;
+}
+
+template <int G, int K>
+__global__ void __launch_bounds__(DxAccCfg<G, K>::THREADS, 1)
+tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmW, const DxAccParams p) {
+  using C = DxAccCfg<G, K>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t sbase = smem_u32(smem);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
+  uint64_t* full = bars;                    // [NST] TMA (tx) -> MMA
+  uint64_t* empty = bars + C::NST;          // [NST] MMA commit -> TMA
+  uint64_t* t_full = bars + 2 * C::NST;     // [2]   MMA commit -> epilogue
+  uint64_t* t_empty = t_full + 2;           // [2]   16 epilogue warps -> MMA
+  uint64_t* d_full = t_empty + 2;           // [RD]  aux warp -> epilogue (destination lists ready)
+  uint64_t* d_empty = d_full + C::RD;       // [RD]  16 epilogue warps -> aux warp
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int bt = blockIdx.x % p.NT, stripe = blockIdx.x / p.NT;
+  const int n_my = p.NG > stripe ? (int)((p.NG - stripe + p.S - 1) / p.S) : 0;
+  const int NS = p.f2 - p.f1;               // shared-memory accumulator rows in use; row NS is the dummy
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4 * C::NSET); }
+    for (int i = 0; i < C::RD; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_empty[i], 4 * C::NSET); }
+    fence_barrier_init();
+  }
+  if (warp == 4 * C::NSET + 1 && lane == 0) { tma_prefetch_desc(&tmY); tma_prefetch_desc(&tmW); }
+  if (warp == 4 * C::NSET) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 4 * C::NSET + 1) {
+    // ===================== TMA loader: dY tile + W_g =====================
+    if (lane == 0) {
+      for (int i = 0; i < n_my; ++i) {
+        const int64_t g = stripe + (int64_t)i * p.S;
+        const int st = i % C::NST;
+        mbar_wait(&empty[st], ((i / C::NST) & 1) ^ 1);
+        mbar_arrive_expect_tx(&full[st], C::STAGE);
+        uint8_t* s0 = smem + st * C::STAGE;
+#pragma unroll
+        for (int kb = 0; kb < G / 64; ++kb) tma_load_3d(s0 + kb * 16384, &tmY, &full[st], kb * 64, bt * 128, (int)g);
+#pragma unroll
+        for (int a = 0; a < K / 64; ++a) tma_load_2d(s0 + C::Y_BYTES + a * (G * 128), &tmW, &full[st], a * 64, (int)(g * G));
+      }
+    }
+  } else if (warp == 4 * C::NSET) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = make_idesc_bf16(128, K, /*A (dY) K-major*/ 0, /*B (W) MN-major*/ 1);
+      for (int i = 0; i < n_my; ++i) {
+        const int st = i % C::NST, slot = i & 1;
+        mbar_wait(&full[st], (i / C::NST) & 1);
+        mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t y0 = sbase + st * C::STAGE, w0 = y0 + C::Y_BYTES;
+        const uint32_t d = tmem_base + slot * K;
+#pragma unroll
+        for (int j = 0; j < G / 16; ++j) {
+          const uint64_t ad = make_sdesc_sw128(y0 + (j >> 2) * 16384 + (j & 3) * 32, 16, 1024);
+          const uint64_t bd = make_sdesc_sw128(w0 + j * 2048, G * 128, 1024);
+          umma_f16(d, ad, bd, idesc, j ? 1u : 0u);
+        }
+        umma_commit(&empty[st]);
+        umma_commit(&t_full[slot]);
+      }
+    }
+  } else if (warp == 4 * C::NSET + 2) {
+    // ===================== auxiliary warp: idx_g -> one destination list per class =====================
+    constexpr int PER = K / 32;
+    int e[PER], en[PER];
+#pragma unroll
+    for (int t = 0; t < PER; ++t) { e[t] = 0; en[t] = 0; }
+    if (n_my > 0) {
+#pragma unroll
+      for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (int64_t)stripe * K + lane * PER + t);
+    }
+    for (int i = 0; i < n_my; ++i) {
+      const int64_t g = stripe + (int64_t)i * p.S;
+      const int r = i % C::RD;
+#pragma unroll
+      for (int t = 0; t < PER; ++t) e[t] = en[t];
+      if (i + 1 < n_my) {
+#pragma unroll
+        for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (g + p.S) * K + lane * PER + t);
+      }
+      // strictly increasing?  class boundaries as slot counts
+      int nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
+      if (lane == 31) nxt = 0x7fffffff;
+      bool inc = e[PER - 1] < nxt;
+#pragma unroll
+      for (int t = 0; t + 1 < PER; ++t) inc &= e[t] < e[t + 1];
+      const bool strict = __all_sync(0xffffffffu, inc);
+      int ca = 0, c1 = 0, cb = 0, c2 = 0;
+#pragma unroll
+      for (int t = 0; t < PER; ++t) { ca += e[t] < p.fa; c1 += e[t] < p.f1; cb += e[t] < p.fb; c2 += e[t] < p.f2; }
+      ca = __reduce_add_sync(0xffffffffu, ca); c1 = __reduce_add_sync(0xffffffffu, c1);
+      cb = __reduce_add_sync(0xffffffffu, cb); c2 = __reduce_add_sync(0xffffffffu, c2);
+      if (!strict) { ca = 0; c1 = 0; cb = 0; c2 = 0; }
+      // list l: slots [lo_l, lo_l + n_l); order of lists = sets 0..3 (TA, SB, TC, SD), then L
+      const int lo[C::NLIST] = {0, c1, ca, cb, c2};
+      const int nn[C::NLIST] = {ca, cb - c1, c1 - ca, c2 - cb, K - c2};
+      mbar_wait(&d_empty[r], ((i / C::RD) & 1) ^ 1);
+      const uint32_t ring = sbase + C::OFF_RING + r * C::RING_BYTES;
+      const uint32_t sidx = ring + C::RING_META, lists = sidx + K * 4;
+#pragma unroll
+      for (int t = 0; t < PER; ++t) sts32(sidx + (lane * PER + t) * 4, (uint32_t)e[t]);
+      if (lane == 0) {
+#pragma unroll
+        for (int l = 0; l < C::NLIST; ++l) { sts32(ring + l * 4, (uint32_t)lo[l]); sts32(ring + 32 + l * 4, (uint32_t)nn[l]); }
+      }
+      __syncwarp();
+#pragma unroll
+      for (int l = 0; l < C::NLIST; ++l) {
+        for (int k = lane; k < C::LIST_LEN; k += 32) {
+          const bool real = k < nn[l];
+          const int f = real ? dxa_lds32i(sidx + (lo[l] + k) * 4) : 0;
+          int code;
+          if (l == 0 || l == 2) code = real ? 2 * K + f : C::TDUMMY;                 // TMEM column
+          else if (l == 1 || l == 3) code = (real ? f - p.f1 : NS) * 512;            // byte offset of the accumulator row
+          else code = f * p.Bpad;                                                    // element offset of the dX^T row (padding is never used)
+          sts32(lists + (l * C::LIST_LEN + k) * 4, (uint32_t)code);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&d_full[r]);
+    }
+  } else {
+    // ===================== epilogue: set = class owner, q = TMEM lane quadrant, lane = batch row =====================
+    const int set = warp >> 2, q = warp & 3;
+    const bool is_t = (set & 1) == 0;                                        // sets 0, 2: TMEM classes; 1, 3: shared memory
+    const int row = q * 32 + lane;
+    const int b = bt * 128 + row;
+    const bool vb = b < p.B;
+    const uint32_t tlane = tmem_base + ((uint32_t)(q * 32) << 16);
+    const uint32_t sown = sbase + C::OFF_ACC + row * 4;                      // + accumulator row * 512
+    float* const gcol = p.dXt + b;                                           // + f * Bpad
+    // this set's own accumulators: [c_lo, c_hi) TMEM columns (relative to the lane base) or shared-memory rows
+    const int c_lo = set == 0 ? 2 * K : set == 2 ? 2 * K + p.fa : set == 1 ? 0 : p.fb - p.f1;
+    const int c_hi = set == 0 ? 2 * K + p.fa : set == 2 ? 2 * K + p.f1 : set == 1 ? p.fb - p.f1 : NS;
+    if (is_t) {
+      for (int c = c_lo; c < c_hi; ++c) dxa_tst1(tlane + c, 0u);
+      dxa_tmem_st_wait();
+    } else {
+      for (int r = c_lo; r < c_hi; ++r) dxa_sts32f(sown + r * 512, 0.f);
+    }
+    for (int i = 0; i < n_my; ++i) {
+      const int r = i % C::RD, slot = i & 1;
+      mbar_wait(&d_full[r], (i / C::RD) & 1);
+      const uint32_t ring = sbase + C::OFF_RING + r * C::RING_BYTES;
+      const uint32_t lists = ring + C::RING_META + K * 4;
+      const int lo_s = dxa_lds32i(ring + set * 4), n_s = dxa_lds32i(ring + 32 + set * 4);
+      const int lo_l = dxa_lds32i(ring + C::NSET * 4), n_l = dxa_lds32i(ring + 32 + C::NSET * 4);
+      mbar_wait(&t_full[slot], (i >> 1) & 1);
+      tc_fence_after();
+      const uint32_t tp = tlane + slot * K;
+      if (is_t) {
+        dxa_tmem_st_wait();                                   // the previous group's stores to these columns have landed
+#pragma unroll 1
+        for (int m = 0; m * 16 < n_s; ++m) {
+          uint32_t pv[16], a[16];
+          int dst[16];
+          tmem_ld16(tp + lo_s + m * 16, pv);
+          dxa_load_dest(lists + (set * C::LIST_LEN + m * 16) * 4, dst);
+#pragma unroll
+          for (int u = 0; u < 16; ++u) a[u] = dxa_tld1(tlane + dst[u]);
+          tmem_ld_wait();
+#pragma unroll
+          for (int u = 0; u < 16; ++u) dxa_tst1(tlane + dst[u], __float_as_uint(__uint_as_float(a[u]) + __uint_as_float(pv[u])));
+        }
+      } else {
+#pragma unroll 1
+        for (int m = 0; m * 16 < n_s; ++m) {
+          uint32_t pv[16];
+          float a[16];
+          int dst[16];
+          tmem_ld16(tp + lo_s + m * 16, pv);
+          dxa_load_dest(lists + (set * C::LIST_LEN + m * 16) * 4, dst);
+#pragma unroll
+          for (int u = 0; u < 16; ++u) a[u] = dxa_lds32f(sown + dst[u]);
+          tmem_ld_wait();
+#pragma unroll
+          for (int u = 0; u < 16; ++u) dxa_sts32f(sown + dst[u], a[u] + __uint_as_float(pv[u]));
+        }
+      }
+      // the L class: chunks dealt round-robin to the sets (red.global is atomic, no ownership needed)
+#pragma unroll 1
+      for (int m = set; m * 16 < n_l; m += C::NSET) {
+        uint32_t pv[16];
+        int dst[16];
+        tmem_ld16(tp + lo_l + m * 16, pv);
+        dxa_load_dest(lists + (C::NSET * C::LIST_LEN + m * 16) * 4, dst);
+        tmem_ld_wait();
+        // no dummy target here: a shared dummy word in L2 would serialise the reductions of every CTA on one address
+        if (vb) {
+          if (m * 16 + 16 <= n_l) {
+#pragma unroll
+            for (int u = 0; u < 16; ++u) dxa_red_add_f32(gcol + dst[u], __uint_as_float(pv[u]));
+          } else {
+#pragma unroll
+            for (int u = 0; u < 16; ++u)
+              if (m * 16 + u < n_l) dxa_red_add_f32(gcol + dst[u], __uint_as_float(pv[u]));
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) { mbar_arrive(&t_empty[slot]); mbar_arrive(&d_empty[r]); }
+    }
+    // flush this thread's accumulators (its batch row of every feature this set owns) into dX^T
+    if (is_t) {
+      dxa_tmem_st_wait();
+      for (int c0 = c_lo; c0 < c_hi; c0 += 16) {
+        uint32_t v[16];
+        tmem_ld16(tlane + c0, v);            // may read past c_hi: still inside the 512 allocated columns
+        tmem_ld_wait();
+        if (vb) {
+#pragma unroll
+          for (int u = 0; u < 16; ++u)
+            if (c0 + u < c_hi) dxa_red_add_f32(gcol + (size_t)(c0 + u - 2 * K) * p.Bpad, __uint_as_float(v[u]));
+        }
+      }
+    } else if (vb) {
+      for (int r = c_lo; r < c_hi; ++r) dxa_red_add_f32(gcol + (size_t)(p.f1 + r) * p.Bpad, dxa_lds32f(sown + r * 512));
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 4 * C::NSET) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
+}
+
+template <int G, int K>
+static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
+                         cudaStream_t st) {
+  using C = DxAccCfg<G, K>;
+  CUtensorMap tmY, tmW;
+  {
+    const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
+    const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
+    const uint32_t box[3] = {64, 128, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, 128);
+    if (rc) return rc;
+  }
+  {
+    const uint64_t dims[2] = {(uint64_t)K, (uint64_t)sh.L};
+    const uint64_t str[1] = {(uint64_t)K * 2};
+    const uint32_t box[2] = {64, (uint32_t)G};
+    int rc = encode_tmap(&tmW, 2, W, 2, dims, str, box, 128);
+    if (rc) return rc;
+  }
+  DxAccParams p;
+  p.dXt = dXt; p.idx = idx; p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NG = sh.NG; p.d = sh.d;
+  if (p.NT > s->num_sms) return HASTE_ERR_UNSUPPORTED;
+  if ((int64_t)sh.d * sh.Bpad > 0x7fffffff) return HASTE_ERR_UNSUPPORTED;   // list codes are 32-bit element offsets
+  p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NT));
+  // class sizes: what fits (tuning knobs for experiments: HASTE_DX_F1, HASTE_DX_NS)
+  int f1 = std::min(sh.d, C::TF), ns = C::NS_MAX;
+  if (const char* e = getenv("HASTE_DX_F1")) f1 = std::max(0, std::min(f1, atoi(e)));
+  if (const char* e = getenv("HASTE_DX_NS")) ns = std::max(0, std::min(ns, atoi(e)));
+  ns = std::min(ns, sh.d - f1);
+  p.f1 = f1; p.fa = f1 / 2; p.f2 = f1 + ns; p.fb = f1 + ns / 2;
+  const int smem = C::OFF_ACC + (ns + 1) * 512 + 1024;
+  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  tc_dx_acc_kernel<G, K><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
+                   cudaStream_t st) {
+#define HASTE_DXA(G_, K_) if (sh.G == G_ && sh.K == K_) return launch_dx_acc<G_, K_>(s, sh, idx, W, dY, dXt, st)
+  HASTE_DXA(64, 128); HASTE_DXA(64, 64); HASTE_DXA(128, 64); HASTE_DXA(128, 128);
+#undef HASTE_DXA
+  return HASTE_ERR_UNSUPPORTED;
+}
+
+}  // namespace haste
