@@ -15,7 +15,7 @@
 //     L  = [f2, d)                   red.global.add.f32 into dX^T, as in the first version (tc_dx.cu)
 // A CTA owns (128-row batch tile, stripe of groups).  Per group: TMA loads the dY tile and W_g, one thread
 // issues P^T[128 batch x K slots] = dY tile * W_g (tcgen05, fp32 in TMEM, double buffered), an auxiliary
-// warp turns idx_g into one destination list per class, and 16 epilogue warps (4 sets x 4 TMEM lane
+// warp (one of four, round-robin) turns idx_g into one destination list per class, and 16 epilogue warps (4 sets x 4 TMEM lane
 // quadrants; a lane owns one batch row) add column j of P into the destination of slot j.  Set s owns class s
 // exclusively, so no two threads ever touch the same accumulator word and nothing on chip is atomic; the L
 // chunks are dealt round-robin to the four sets (they are atomic in L2).  Lists are padded to whole chunks with
@@ -47,13 +47,13 @@ template <int G, int K> struct DxAccCfg {
   static constexpr int Y_BYTES = G * 256;                     // [G/64 k-blocks][128 batch rows][128 B]
   static constexpr int W_BYTES = G * K * 2;                   // [K/64 slot atoms][G label rows][128 B]
   static constexpr int STAGE = Y_BYTES + W_BYTES;
-  static constexpr int NST = STAGE <= 32768 ? 3 : 2;
+  static constexpr int NST = 2;
   static constexpr int LIST_LEN = K + 16;                     // entries per list (padding for the last chunk)
   static constexpr int RING_META = 64;                        // lo[5], n[5]
   static constexpr int RING_BYTES = (RING_META + K * 4 + NLIST * LIST_LEN * 4 + 127) / 128 * 128;
   static constexpr int RD = 4;                                // depth of the destination-list ring
-  static constexpr int TF = 512 - 2 * K - 16;                 // TMEM accumulator columns usable by features
-  static constexpr int TDUMMY = 2 * K + TF;                   // dummy TMEM column (first of the 16 spare ones)
+  static constexpr int TF = 512 - 2 * K - 1;                  // TMEM accumulator columns usable by features
+  static constexpr int TDUMMY = 511;                          // dummy TMEM column
   static constexpr int OFF_RING = NST * STAGE;
   static constexpr int OFF_BAR = OFF_RING + RD * RING_BYTES;
   static constexpr int NBAR = 2 * NST + 4 + 2 * RD;
@@ -61,7 +61,8 @@ template <int G, int K> struct DxAccCfg {
   static constexpr int OFF_ACC = (OFF_MISC + 64 + 511) / 512 * 512;
   static constexpr int NS_MAX = (232448 - 1024 - OFF_ACC) / 512 - 1;   // shared-memory accumulator rows (+1 dummy row)
   static_assert(NS_MAX >= 16, "no room for shared-memory accumulators");
-  static constexpr int THREADS = (4 * NSET + 3) * 32;
+  static constexpr int NAUX = RD;                             // list-building warps: warp a owns ring slot a (groups i = a mod RD)
+  static constexpr int THREADS = (4 * NSET + 2 + NAUX) * 32;
 };
 
 __device__ __forceinline__ void dxa_red_add_f32(float* addr, float v) {
@@ -94,11 +95,50 @@ __device__ __forceinline__ float dxa_lds32f(uint32_t addr) {
 __device__ __forceinline__ void dxa_sts32f(uint32_t addr, float v) {
   asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
-// 16 destination codes of one chunk of a list
-__device__ __forceinline__ void dxa_load_dest(uint32_t addr, int (&dst)[16]) {
-  const int4 a0 = dxa_lds128i(addr), a1 = dxa_lds128i(addr + 16), a2 = dxa_lds128i(addr + 32), a3 = dxa_lds128i(addr + 48);
-  dst[0] = a0.x; dst[1] = a0.y; dst[2] = a0.z; dst[3] = a0.w; dst[4] = a1.x; dst[5] = a1.y; dst[6] = a1.z; dst[7] = a1.w;
-  dst[8] = a2.x; dst[9] = a2.y; dst[10] = a2.z; dst[11] = a2.w; dst[12] = a3.x; dst[13] = a3.y; dst[14] = a3.z; dst[15] = a3.w;
+__device__ __forceinline__ void dxa_red_add_f32(const char* addr, float v) {
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void dxa_tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
+}
+template <int N> __device__ __forceinline__ void dxa_tmem_ldn(uint32_t taddr, uint32_t (&v)[N]);
+template <> __device__ __forceinline__ void dxa_tmem_ldn<16>(uint32_t taddr, uint32_t (&v)[16]) { tmem_ld16(taddr, v); }
+template <> __device__ __forceinline__ void dxa_tmem_ldn<8>(uint32_t taddr, uint32_t (&v)[8]) { dxa_tmem_ld8(taddr, v); }
+// N destination codes of one chunk of a list (16-byte aligned)
+template <int N> __device__ __forceinline__ void dxa_load_dest(uint32_t addr, int (&dst)[N]) {
+#pragma unroll
+  for (int i = 0; i < N / 4; ++i) {
+    const int4 a = dxa_lds128i(addr + i * 16);
+    dst[4 * i] = a.x; dst[4 * i + 1] = a.y; dst[4 * i + 2] = a.z; dst[4 * i + 3] = a.w;
+  }
+}
+// one chunk of N slots of a TMEM class: acc column dst[u] += P column u (both in this warp's lane quadrant)
+template <int N> __device__ __forceinline__ void dxa_chunk_t(uint32_t tp, uint32_t lst, uint32_t tlane) {
+  uint32_t pv[N], a[N];
+  int dst[N];
+  dxa_tmem_ldn<N>(tp, pv);
+  dxa_load_dest<N>(lst, dst);
+#pragma unroll
+  for (int u = 0; u < N; ++u) a[u] = dxa_tld1(tlane + dst[u]);
+  tmem_ld_wait();
+#pragma unroll
+  for (int u = 0; u < N; ++u) dxa_tst1(tlane + dst[u], __float_as_uint(__uint_as_float(a[u]) + __uint_as_float(pv[u])));
+}
+// one chunk of N slots of a shared-memory class: acc row (byte offset dst[u]), this thread's word += P column u
+template <int N> __device__ __forceinline__ void dxa_chunk_s(uint32_t tp, uint32_t lst, uint32_t sown) {
+  uint32_t pv[N];
+  float a[N];
+  int dst[N];
+  dxa_tmem_ldn<N>(tp, pv);
+  dxa_load_dest<N>(lst, dst);
+#pragma unroll
+  for (int u = 0; u < N; ++u) a[u] = dxa_lds32f(sown + dst[u]);
+  tmem_ld_wait();
+#pragma unroll
+  for (int u = 0; u < N; ++u) dxa_sts32f(sown + dst[u], a[u] + __uint_as_float(pv[u]));
 }
 
 template <int G, int K>
@@ -171,24 +211,26 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         umma_commit(&t_full[slot]);
       }
     }
-  } else if (warp == 4 * C::NSET + 2) {
-    // ===================== auxiliary warp: idx_g -> one destination list per class =====================
+  } else if (warp >= 4 * C::NSET + 2) {
+    // ===================== auxiliary warps: idx_g -> one destination list per class =====================
+    // (one warp per ring slot: building the lists of a group is a ~1 us latency chain, longer than a group's epilogue)
     constexpr int PER = K / 32;
+    const int aw = warp - (4 * C::NSET + 2);
     int e[PER], en[PER];
 #pragma unroll
     for (int t = 0; t < PER; ++t) { e[t] = 0; en[t] = 0; }
-    if (n_my > 0) {
+    if (aw < n_my) {
 #pragma unroll
-      for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (int64_t)stripe * K + lane * PER + t);
+      for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (stripe + (int64_t)aw * p.S) * K + lane * PER + t);
     }
-    for (int i = 0; i < n_my; ++i) {
+    for (int i = aw; i < n_my; i += C::NAUX) {
       const int64_t g = stripe + (int64_t)i * p.S;
-      const int r = i % C::RD;
+      const int r = aw;
 #pragma unroll
       for (int t = 0; t < PER; ++t) e[t] = en[t];
-      if (i + 1 < n_my) {
+      if (i + C::NAUX < n_my) {
 #pragma unroll
-        for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (g + p.S) * K + lane * PER + t);
+        for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (g + (int64_t)C::NAUX * p.S) * K + lane * PER + t);
       }
       // strictly increasing?  class boundaries as slot counts
       int nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
@@ -216,18 +258,29 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         for (int l = 0; l < C::NLIST; ++l) { sts32(ring + l * 4, (uint32_t)lo[l]); sts32(ring + 32 + l * 4, (uint32_t)nn[l]); }
       }
       __syncwarp();
+      // all gathers first, then all stores: one warp builds every list, so its latency chain is the critical path
+      constexpr int NIT = (C::LIST_LEN + 31) / 32;
+      int fv[C::NLIST][NIT];
 #pragma unroll
-      for (int l = 0; l < C::NLIST; ++l) {
-        for (int k = lane; k < C::LIST_LEN; k += 32) {
+      for (int l = 0; l < C::NLIST; ++l)
+#pragma unroll
+        for (int t = 0; t < NIT; ++t) {
+          const int k = lane + 32 * t;
+          fv[l][t] = dxa_lds32i(sidx + (min(lo[l] + k, K - 1)) * 4);
+        }
+#pragma unroll
+      for (int l = 0; l < C::NLIST; ++l)
+#pragma unroll
+        for (int t = 0; t < NIT; ++t) {
+          const int k = lane + 32 * t;
           const bool real = k < nn[l];
-          const int f = real ? dxa_lds32i(sidx + (lo[l] + k) * 4) : 0;
+          const int f = fv[l][t];
           int code;
           if (l == 0 || l == 2) code = real ? 2 * K + f : C::TDUMMY;                 // TMEM column
           else if (l == 1 || l == 3) code = (real ? f - p.f1 : NS) * 512;            // byte offset of the accumulator row
-          else code = f * p.Bpad;                                                    // element offset of the dX^T row (padding is never used)
-          sts32(lists + (l * C::LIST_LEN + k) * 4, (uint32_t)code);
+          else code = f * p.Bpad * 4;                                                // byte offset of the dX^T row (padding is never used)
+          if (k < C::LIST_LEN) sts32(lists + (l * C::LIST_LEN + k) * 4, (uint32_t)code);
         }
-      }
       __syncwarp();
       if (lane == 0) mbar_arrive(&d_full[r]);
     }
@@ -241,6 +294,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     const uint32_t tlane = tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t sown = sbase + C::OFF_ACC + row * 4;                      // + accumulator row * 512
     float* const gcol = p.dXt + b;                                           // + f * Bpad
+    const char* const gbytes = reinterpret_cast<const char*>(gcol);          // + byte offset of the dX^T row (L list code)
     // this set's own accumulators: [c_lo, c_hi) TMEM columns (relative to the lane base) or shared-memory rows
     const int c_lo = set == 0 ? 2 * K : set == 2 ? 2 * K + p.fa : set == 1 ? 0 : p.fb - p.f1;
     const int c_hi = set == 0 ? 2 * K + p.fa : set == 2 ? 2 * K + p.f1 : set == 1 ? p.fb - p.f1 : NS;
@@ -260,52 +314,37 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
       mbar_wait(&t_full[slot], (i >> 1) & 1);
       tc_fence_after();
       const uint32_t tp = tlane + slot * K;
+      const uint32_t lst = lists + set * C::LIST_LEN * 4;
       if (is_t) {
         dxa_tmem_st_wait();                                   // the previous group's stores to these columns have landed
+        int m = 0;
 #pragma unroll 1
-        for (int m = 0; m * 16 < n_s; ++m) {
-          uint32_t pv[16], a[16];
-          int dst[16];
-          tmem_ld16(tp + lo_s + m * 16, pv);
-          dxa_load_dest(lists + (set * C::LIST_LEN + m * 16) * 4, dst);
-#pragma unroll
-          for (int u = 0; u < 16; ++u) a[u] = dxa_tld1(tlane + dst[u]);
-          tmem_ld_wait();
-#pragma unroll
-          for (int u = 0; u < 16; ++u) dxa_tst1(tlane + dst[u], __float_as_uint(__uint_as_float(a[u]) + __uint_as_float(pv[u])));
-        }
+        for (; n_s - m > 8; m += 16) dxa_chunk_t<16>(tp + lo_s + m, lst + m * 4, tlane);
+        if (n_s - m > 0) dxa_chunk_t<8>(tp + lo_s + m, lst + m * 4, tlane);
       } else {
+        int m = 0;
 #pragma unroll 1
-        for (int m = 0; m * 16 < n_s; ++m) {
-          uint32_t pv[16];
-          float a[16];
-          int dst[16];
-          tmem_ld16(tp + lo_s + m * 16, pv);
-          dxa_load_dest(lists + (set * C::LIST_LEN + m * 16) * 4, dst);
-#pragma unroll
-          for (int u = 0; u < 16; ++u) a[u] = dxa_lds32f(sown + dst[u]);
-          tmem_ld_wait();
-#pragma unroll
-          for (int u = 0; u < 16; ++u) dxa_sts32f(sown + dst[u], a[u] + __uint_as_float(pv[u]));
-        }
+        for (; n_s - m > 8; m += 16) dxa_chunk_s<16>(tp + lo_s + m, lst + m * 4, sown);
+        if (n_s - m > 0) dxa_chunk_s<8>(tp + lo_s + m, lst + m * 4, sown);
       }
-      // the L class: chunks dealt round-robin to the sets (red.global is atomic, no ownership needed)
+      // the L class: chunks dealt round-robin to the sets (red.global is atomic, no ownership needed).  No dummy
+      // target here: a shared dummy word in L2 would serialise the reductions of every CTA on one address.
+      const uint32_t lstl = lists + C::NSET * C::LIST_LEN * 4;
 #pragma unroll 1
-      for (int m = set; m * 16 < n_l; m += C::NSET) {
+      for (int m = set * 16; m < n_l; m += C::NSET * 16) {
         uint32_t pv[16];
         int dst[16];
-        tmem_ld16(tp + lo_l + m * 16, pv);
-        dxa_load_dest(lists + (C::NSET * C::LIST_LEN + m * 16) * 4, dst);
+        tmem_ld16(tp + lo_l + m, pv);
+        dxa_load_dest<16>(lstl + m * 4, dst);
         tmem_ld_wait();
-        // no dummy target here: a shared dummy word in L2 would serialise the reductions of every CTA on one address
         if (vb) {
-          if (m * 16 + 16 <= n_l) {
+          if (m + 16 <= n_l) {
 #pragma unroll
-            for (int u = 0; u < 16; ++u) dxa_red_add_f32(gcol + dst[u], __uint_as_float(pv[u]));
+            for (int u = 0; u < 16; ++u) dxa_red_add_f32(gbytes + (uint32_t)dst[u], __uint_as_float(pv[u]));
           } else {
 #pragma unroll
             for (int u = 0; u < 16; ++u)
-              if (m * 16 + u < n_l) dxa_red_add_f32(gcol + dst[u], __uint_as_float(pv[u]));
+              if (m + u < n_l) dxa_red_add_f32(gbytes + (uint32_t)dst[u], __uint_as_float(pv[u]));
           }
         }
       }
@@ -318,7 +357,8 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
       dxa_tmem_st_wait();
       for (int c0 = c_lo; c0 < c_hi; c0 += 16) {
         uint32_t v[16];
-        tmem_ld16(tlane + c0, v);            // may read past c_hi: still inside the 512 allocated columns
+#pragma unroll
+        for (int u = 0; u < 16; ++u) v[u] = dxa_tld1(tlane + min(c0 + u, 511));
         tmem_ld_wait();
         if (vb) {
 #pragma unroll
@@ -358,7 +398,7 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   DxAccParams p;
   p.dXt = dXt; p.idx = idx; p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NG = sh.NG; p.d = sh.d;
   if (p.NT > s->num_sms) return HASTE_ERR_UNSUPPORTED;
-  if ((int64_t)sh.d * sh.Bpad > 0x7fffffff) return HASTE_ERR_UNSUPPORTED;   // list codes are 32-bit element offsets
+  if ((int64_t)sh.d * sh.Bpad * 4 > 0x7fffffff) return HASTE_ERR_UNSUPPORTED;   // list codes are 32-bit byte offsets
   p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NT));
   // class sizes: what fits (tuning knobs for experiments: HASTE_DX_F1, HASTE_DX_NS)
   int f1 = std::min(sh.d, C::TF), ns = C::NS_MAX;
