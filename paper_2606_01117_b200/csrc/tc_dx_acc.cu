@@ -18,7 +18,8 @@
 // warp (one of four, round-robin) turns idx_g into one destination list per class, and 16 epilogue warps (4 sets x 4 TMEM lane
 // quadrants; a lane owns one batch row) add column j of P into the destination of slot j.  Set s owns class s
 // exclusively, so no two threads ever touch the same accumulator word and nothing on chip is atomic; the L
-// chunks are dealt round-robin to the four sets (they are atomic in L2).  Lists are padded to whole chunks with
+// chunks (atomic in L2, hence owner-free) are dealt round-robin to the four sets, shared-memory sets first
+// (handing them out dynamically through a shared-memory counter was measured slower: 0.319 vs 0.298 ms).  Lists are padded to whole chunks with
 // a dummy destination per class (a spare TMEM column, a spare shared-memory row), so the on-chip
 // inner loops carry no predicates; only the last L chunk is predicated (a dummy word in L2 would be one address
 // hammered by every CTA).  Groups whose idx row is not strictly increasing (duplicates, unsorted:
@@ -41,16 +42,16 @@ struct DxAccParams {
   int fa, f1, fb, f2;   // class boundaries (see above)
 };
 
-template <int G, int K> struct DxAccCfg {
+template <int G, int K, int NST_> struct DxAccCfg {
   static constexpr int NSET = 4;                              // epilogue sets: 0 = TA, 1 = SB, 2 = TC, 3 = SD
   static constexpr int NLIST = NSET + 1;                      // + the L list
   static constexpr int Y_BYTES = G * 256;                     // [G/64 k-blocks][128 batch rows][128 B]
   static constexpr int W_BYTES = G * K * 2;                   // [K/64 slot atoms][G label rows][128 B]
   static constexpr int STAGE = Y_BYTES + W_BYTES;
-  static constexpr int NST = 2;
+  static constexpr int NST = NST_;                            // operand stages (dY tile + W_g) in flight
   static constexpr int LIST_LEN = K + 16;                     // entries per list (padding for the last chunk)
-  static constexpr int RING_META = 64;                        // lo[5], n[5]
-  static constexpr int RING_BYTES = (RING_META + K * 4 + NLIST * LIST_LEN * 4 + 127) / 128 * 128;
+  static constexpr int RING_META = 48;                        // lo[5] at 0, n[5] at 20
+  static constexpr int RING_BYTES = (RING_META + NLIST * LIST_LEN * 4 + 127) / 128 * 128;
   static constexpr int RD = 4;                                // depth of the destination-list ring
   static constexpr int TF = 512 - 2 * K - 1;                  // TMEM accumulator columns usable by features
   static constexpr int TDUMMY = 511;                          // dummy TMEM column
@@ -60,8 +61,8 @@ template <int G, int K> struct DxAccCfg {
   static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;
   static constexpr int OFF_ACC = (OFF_MISC + 64 + 511) / 512 * 512;
   static constexpr int NS_MAX = (232448 - 1024 - OFF_ACC) / 512 - 1;   // shared-memory accumulator rows (+1 dummy row)
-  static_assert(NS_MAX >= 16, "no room for shared-memory accumulators");
-  static constexpr int NAUX = RD;                             // list-building warps: warp a owns ring slot a (groups i = a mod RD)
+  static constexpr bool FITS = NS_MAX >= 64;                  // otherwise use fewer stages
+  static constexpr int NAUX = 2;                              // list-building warps: warp a builds the lists of groups i = a mod NAUX
   static constexpr int THREADS = (4 * NSET + 2 + NAUX) * 32;
 };
 
@@ -107,6 +108,10 @@ __device__ __forceinline__ void dxa_tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
 template <int N> __device__ __forceinline__ void dxa_tmem_ldn(uint32_t taddr, uint32_t (&v)[N]);
 template <> __device__ __forceinline__ void dxa_tmem_ldn<16>(uint32_t taddr, uint32_t (&v)[16]) { tmem_ld16(taddr, v); }
 template <> __device__ __forceinline__ void dxa_tmem_ldn<8>(uint32_t taddr, uint32_t (&v)[8]) { dxa_tmem_ld8(taddr, v); }
+template <> __device__ __forceinline__ void dxa_tmem_ldn<24>(uint32_t taddr, uint32_t (&v)[24]) {
+  tmem_ld16(taddr, reinterpret_cast<uint32_t(&)[16]>(v[0]));
+  dxa_tmem_ld8(taddr + 16, reinterpret_cast<uint32_t(&)[8]>(v[16]));
+}
 // N destination codes of one chunk of a list (16-byte aligned)
 template <int N> __device__ __forceinline__ void dxa_load_dest(uint32_t addr, int (&dst)[N]) {
 #pragma unroll
@@ -141,10 +146,15 @@ template <int N> __device__ __forceinline__ void dxa_chunk_s(uint32_t tp, uint32
   for (int u = 0; u < N; ++u) dxa_sts32f(sown + dst[u], a[u] + __uint_as_float(pv[u]));
 }
 
-template <int G, int K>
-__global__ void __launch_bounds__(DxAccCfg<G, K>::THREADS, 1)
+// 20 warps poll barriers here; a polling loop costs issue slots the working warps need, so back off between polls
+template <int NS_SLEEP> __device__ __forceinline__ void dxa_wait(uint64_t* bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) __nanosleep(NS_SLEEP);
+}
+
+template <int G, int K, int NST>
+__global__ void __launch_bounds__(DxAccCfg<G, K, NST>::THREADS, 1)
 tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmW, const DxAccParams p) {
-  using C = DxAccCfg<G, K>;
+  using C = DxAccCfg<G, K, NST>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const uint32_t sbase = smem_u32(smem);
@@ -213,7 +223,8 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     }
   } else if (warp >= 4 * C::NSET + 2) {
     // ===================== auxiliary warps: idx_g -> one destination list per class =====================
-    // (one warp per ring slot: building the lists of a group is a ~1 us latency chain, longer than a group's epilogue)
+    // Lane holds slots j = lane + 32 t.  Slot j belongs to the class whose slot range contains it and is entry
+    // j - lo of that class's list, so every lane writes its own PER entries; no gather, no second pass.
     constexpr int PER = K / 32;
     const int aw = warp - (4 * C::NSET + 2);
     int e[PER], en[PER];
@@ -221,66 +232,62 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     for (int t = 0; t < PER; ++t) { e[t] = 0; en[t] = 0; }
     if (aw < n_my) {
 #pragma unroll
-      for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (stripe + (int64_t)aw * p.S) * K + lane * PER + t);
+      for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (stripe + (int64_t)aw * p.S) * K + lane + 32 * t);
     }
     for (int i = aw; i < n_my; i += C::NAUX) {
       const int64_t g = stripe + (int64_t)i * p.S;
-      const int r = aw;
+      const int r = i % C::RD;
 #pragma unroll
       for (int t = 0; t < PER; ++t) e[t] = en[t];
       if (i + C::NAUX < n_my) {
 #pragma unroll
-        for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (g + (int64_t)C::NAUX * p.S) * K + lane * PER + t);
+        for (int t = 0; t < PER; ++t) en[t] = __ldg(p.idx + (g + (int64_t)C::NAUX * p.S) * K + lane + 32 * t);
       }
-      // strictly increasing?  class boundaries as slot counts
-      int nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
-      if (lane == 31) nxt = 0x7fffffff;
-      bool inc = e[PER - 1] < nxt;
+      // strictly increasing?  (slot j+1 is the next lane's value, or lane 0's value of the next t)
+      bool inc = true;
 #pragma unroll
-      for (int t = 0; t + 1 < PER; ++t) inc &= e[t] < e[t + 1];
+      for (int t = 0; t < PER; ++t) {
+        int nxt = __shfl_down_sync(0xffffffffu, e[t], 1);
+        const int wrap = __shfl_sync(0xffffffffu, t + 1 < PER ? e[(t + 1) % PER] : 0x7fffffff, 0);
+        if (lane == 31) nxt = wrap;
+        inc &= e[t] < nxt;
+      }
       const bool strict = __all_sync(0xffffffffu, inc);
+      // class boundaries as slot counts
       int ca = 0, c1 = 0, cb = 0, c2 = 0;
 #pragma unroll
       for (int t = 0; t < PER; ++t) { ca += e[t] < p.fa; c1 += e[t] < p.f1; cb += e[t] < p.fb; c2 += e[t] < p.f2; }
       ca = __reduce_add_sync(0xffffffffu, ca); c1 = __reduce_add_sync(0xffffffffu, c1);
       cb = __reduce_add_sync(0xffffffffu, cb); c2 = __reduce_add_sync(0xffffffffu, c2);
       if (!strict) { ca = 0; c1 = 0; cb = 0; c2 = 0; }
-      // list l: slots [lo_l, lo_l + n_l); order of lists = sets 0..3 (TA, SB, TC, SD), then L
-      const int lo[C::NLIST] = {0, c1, ca, cb, c2};
-      const int nn[C::NLIST] = {ca, cb - c1, c1 - ca, c2 - cb, K - c2};
-      mbar_wait(&d_empty[r], ((i / C::RD) & 1) ^ 1);
+      dxa_wait<64>(&d_empty[r], ((i / C::RD) & 1) ^ 1);
       const uint32_t ring = sbase + C::OFF_RING + r * C::RING_BYTES;
-      const uint32_t sidx = ring + C::RING_META, lists = sidx + K * 4;
-#pragma unroll
-      for (int t = 0; t < PER; ++t) sts32(sidx + (lane * PER + t) * 4, (uint32_t)e[t]);
+      const uint32_t lists = ring + C::RING_META;
+      // lists in ring order: sets 0..3 = TA [0,ca), SB [c1,cb), TC [ca,c1), SD [cb,c2); then L [c2,K)
       if (lane == 0) {
-#pragma unroll
-        for (int l = 0; l < C::NLIST; ++l) { sts32(ring + l * 4, (uint32_t)lo[l]); sts32(ring + 32 + l * 4, (uint32_t)nn[l]); }
+        sts32(ring + 0, 0u); sts32(ring + 4, (uint32_t)c1); sts32(ring + 8, (uint32_t)ca); sts32(ring + 12, (uint32_t)cb);
+        sts32(ring + 16, (uint32_t)c2);
+        sts32(ring + 20, (uint32_t)ca); sts32(ring + 24, (uint32_t)(cb - c1)); sts32(ring + 28, (uint32_t)(c1 - ca));
+        sts32(ring + 32, (uint32_t)(c2 - cb)); sts32(ring + 36, (uint32_t)(K - c2));
       }
-      __syncwarp();
-      // all gathers first, then all stores: one warp builds every list, so its latency chain is the critical path
-      constexpr int NIT = (C::LIST_LEN + 31) / 32;
-      int fv[C::NLIST][NIT];
 #pragma unroll
-      for (int l = 0; l < C::NLIST; ++l)
-#pragma unroll
-        for (int t = 0; t < NIT; ++t) {
-          const int k = lane + 32 * t;
-          fv[l][t] = dxa_lds32i(sidx + (min(lo[l] + k, K - 1)) * 4);
-        }
-#pragma unroll
-      for (int l = 0; l < C::NLIST; ++l)
-#pragma unroll
-        for (int t = 0; t < NIT; ++t) {
-          const int k = lane + 32 * t;
-          const bool real = k < nn[l];
-          const int f = fv[l][t];
-          int code;
-          if (l == 0 || l == 2) code = real ? 2 * K + f : C::TDUMMY;                 // TMEM column
-          else if (l == 1 || l == 3) code = (real ? f - p.f1 : NS) * 512;            // byte offset of the accumulator row
-          else code = f * p.Bpad * 4;                                                // byte offset of the dX^T row (padding is never used)
-          if (k < C::LIST_LEN) sts32(lists + (l * C::LIST_LEN + k) * 4, (uint32_t)code);
-        }
+      for (int t = 0; t < PER; ++t) {
+        const int j = lane + 32 * t, f = e[t];
+        int l, k, code;
+        if (j < ca)      { l = 0; k = j;      code = 2 * K + f; }                 // TMEM column
+        else if (j < c1) { l = 2; k = j - ca; code = 2 * K + f; }
+        else if (j < cb) { l = 1; k = j - c1; code = (f - p.f1) * 512; }          // byte offset of the accumulator row
+        else if (j < c2) { l = 3; k = j - cb; code = (f - p.f1) * 512; }
+        else             { l = 4; k = j - c2; code = f * p.Bpad * 4; }            // byte offset of the dX^T row
+        sts32(lists + (l * C::LIST_LEN + k) * 4, (uint32_t)code);
+      }
+      // pad the on-chip lists to a whole chunk with the class's dummy destination
+      if (lane < 16) {
+        sts32(lists + (0 * C::LIST_LEN + ca + lane) * 4, (uint32_t)C::TDUMMY);
+        sts32(lists + (2 * C::LIST_LEN + (c1 - ca) + lane) * 4, (uint32_t)C::TDUMMY);
+        sts32(lists + (1 * C::LIST_LEN + (cb - c1) + lane) * 4, (uint32_t)(NS * 512));
+        sts32(lists + (3 * C::LIST_LEN + (c2 - cb) + lane) * 4, (uint32_t)(NS * 512));
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(&d_full[r]);
     }
@@ -298,6 +305,8 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     // this set's own accumulators: [c_lo, c_hi) TMEM columns (relative to the lane base) or shared-memory rows
     const int c_lo = set == 0 ? 2 * K : set == 2 ? 2 * K + p.fa : set == 1 ? 0 : p.fb - p.f1;
     const int c_hi = set == 0 ? 2 * K + p.fa : set == 2 ? 2 * K + p.f1 : set == 1 ? p.fb - p.f1 : NS;
+    // L chunks go to the shared-memory sets first: their own chunks cost fewer instructions than the TMEM sets'
+    const int l_first = set == 3 ? 0 : set == 1 ? 1 : set == 2 ? 2 : 3;
     if (is_t) {
       for (int c = c_lo; c < c_hi; ++c) dxa_tst1(tlane + c, 0u);
       dxa_tmem_st_wait();
@@ -306,12 +315,12 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     }
     for (int i = 0; i < n_my; ++i) {
       const int r = i % C::RD, slot = i & 1;
-      mbar_wait(&d_full[r], (i / C::RD) & 1);
+      dxa_wait<64>(&d_full[r], (i / C::RD) & 1);
       const uint32_t ring = sbase + C::OFF_RING + r * C::RING_BYTES;
-      const uint32_t lists = ring + C::RING_META + K * 4;
-      const int lo_s = dxa_lds32i(ring + set * 4), n_s = dxa_lds32i(ring + 32 + set * 4);
-      const int lo_l = dxa_lds32i(ring + C::NSET * 4), n_l = dxa_lds32i(ring + 32 + C::NSET * 4);
-      mbar_wait(&t_full[slot], (i >> 1) & 1);
+      const uint32_t lists = ring + C::RING_META;
+      const int lo_s = dxa_lds32i(ring + set * 4), n_s = dxa_lds32i(ring + 20 + set * 4);
+      const int lo_l = dxa_lds32i(ring + C::NSET * 4), n_l = dxa_lds32i(ring + 20 + C::NSET * 4);
+      dxa_wait<64>(&t_full[slot], (i >> 1) & 1);
       tc_fence_after();
       const uint32_t tp = tlane + slot * K;
       const uint32_t lst = lists + set * C::LIST_LEN * 4;
@@ -319,19 +328,24 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         dxa_tmem_st_wait();                                   // the previous group's stores to these columns have landed
         int m = 0;
 #pragma unroll 1
-        for (; n_s - m > 8; m += 16) dxa_chunk_t<16>(tp + lo_s + m, lst + m * 4, tlane);
-        if (n_s - m > 0) dxa_chunk_t<8>(tp + lo_s + m, lst + m * 4, tlane);
+        for (; n_s - m > 24; m += 16) dxa_chunk_t<16>(tp + lo_s + m, lst + m * 4, tlane);
+        // the rest in ONE pass (8, 16 or 24 slots): a chunk is one latency chain, so as few chunks as registers allow
+        if (n_s - m > 16) dxa_chunk_t<24>(tp + lo_s + m, lst + m * 4, tlane);
+        else if (n_s - m > 8) dxa_chunk_t<16>(tp + lo_s + m, lst + m * 4, tlane);
+        else if (n_s - m > 0) dxa_chunk_t<8>(tp + lo_s + m, lst + m * 4, tlane);
       } else {
         int m = 0;
 #pragma unroll 1
-        for (; n_s - m > 8; m += 16) dxa_chunk_s<16>(tp + lo_s + m, lst + m * 4, sown);
-        if (n_s - m > 0) dxa_chunk_s<8>(tp + lo_s + m, lst + m * 4, sown);
+        for (; n_s - m > 24; m += 16) dxa_chunk_s<16>(tp + lo_s + m, lst + m * 4, sown);
+        if (n_s - m > 16) dxa_chunk_s<24>(tp + lo_s + m, lst + m * 4, sown);
+        else if (n_s - m > 8) dxa_chunk_s<16>(tp + lo_s + m, lst + m * 4, sown);
+        else if (n_s - m > 0) dxa_chunk_s<8>(tp + lo_s + m, lst + m * 4, sown);
       }
-      // the L class: chunks dealt round-robin to the sets (red.global is atomic, no ownership needed).  No dummy
+      // the L class: red.global is atomic, so chunks need no owner.  No dummy
       // target here: a shared dummy word in L2 would serialise the reductions of every CTA on one address.
       const uint32_t lstl = lists + C::NSET * C::LIST_LEN * 4;
 #pragma unroll 1
-      for (int m = set * 16; m < n_l; m += C::NSET * 16) {
+      for (int m = l_first * 16; m < n_l; m += C::NSET * 16) {
         uint32_t pv[16];
         int dst[16];
         tmem_ld16(tp + lo_l + m, pv);
@@ -376,10 +390,10 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
   if (warp == 4 * C::NSET) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
 }
 
-template <int G, int K>
+template <int G, int K, int NST>
 static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                          cudaStream_t st) {
-  using C = DxAccCfg<G, K>;
+  using C = DxAccCfg<G, K, NST>;
   CUtensorMap tmY, tmW;
   {
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
@@ -407,16 +421,24 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   ns = std::min(ns, sh.d - f1);
   p.f1 = f1; p.fa = f1 / 2; p.f2 = f1 + ns; p.fb = f1 + ns / 2;
   const int smem = C::OFF_ACC + (ns + 1) * 512 + 1024;
-  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  tc_dx_acc_kernel<G, K><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K, NST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  tc_dx_acc_kernel<G, K, NST><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }
 
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    cudaStream_t st) {
-#define HASTE_DXA(G_, K_) if (sh.G == G_ && sh.K == K_) return launch_dx_acc<G_, K_>(s, sh, idx, W, dY, dXt, st)
-  HASTE_DXA(64, 128); HASTE_DXA(64, 64); HASTE_DXA(128, 64); HASTE_DXA(128, 128);
+  // operand stages: as many as leave room for a useful number of shared-memory accumulator rows
+  static const int nst_env = getenv("HASTE_DX_NST") ? atoi(getenv("HASTE_DX_NST")) : 0;
+#define HASTE_DXA(G_, K_, DEF_)                                                                       \
+  if (sh.G == G_ && sh.K == K_) {                                                                     \
+    const int nst = nst_env ? nst_env : DEF_;                                                         \
+    if constexpr (DxAccCfg<G_, K_, 4>::FITS) if (nst == 4) return launch_dx_acc<G_, K_, 4>(s, sh, idx, W, dY, dXt, st);  \
+    if constexpr (DxAccCfg<G_, K_, 3>::FITS) if (nst == 3) return launch_dx_acc<G_, K_, 3>(s, sh, idx, W, dY, dXt, st);  \
+    return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, st);                                       \
+  }
+  HASTE_DXA(64, 128, 3); HASTE_DXA(64, 64, 3); HASTE_DXA(128, 64, 3); HASTE_DXA(128, 128, 2);
 #undef HASTE_DXA
   return HASTE_ERR_UNSUPPORTED;
 }
