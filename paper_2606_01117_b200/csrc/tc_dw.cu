@@ -151,28 +151,32 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     }
   } else if (warp == 8) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(G, C::N, /*A (dY) MN-major*/ 1, /*B (H^T) K-major*/ 0);
-      int it = 0;
-      for (int i = 0; i < n_my; ++i) {
-        const int slot = i & 1;
-        mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
+    // whole warp waits, one elected lane issues; descriptors are a per-stage base + compile-time offsets (see tc_tail.cu)
+    constexpr uint32_t idesc = make_idesc_bf16(G, C::N, /*A (dY) MN-major*/ 1, /*B (H^T) K-major*/ 0);
+    const uint64_t bdesc0 = make_sdesc_sw128(sbase, 16, 1024);
+    const uint64_t adesc0 = make_sdesc_sw128(sbase + C::H_BYTES, 8192, 1024);
+    int it = 0;
+    for (int i = 0; i < n_my; ++i) {
+      const int slot = i & 1;
+      mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t d = tmem_base + slot * C::TS;
+      for (int kb = 0; kb < p.NKB; ++kb, ++it) {
+        const int st = it % C::NST;
+        mbar_wait(&full[st], (it / C::NST) & 1);
         tc_fence_after();
-        const uint32_t d = tmem_base + slot * C::TS;
-        for (int kb = 0; kb < p.NKB; ++kb, ++it) {
-          const int st = it % C::NST;
-          mbar_wait(&full[st], (it / C::NST) & 1);
-          tc_fence_after();
-          const uint32_t h0 = sbase + st * C::STAGE, y0 = h0 + C::H_BYTES;
+        if (elect_one()) {
+          const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
-            const uint64_t ad = make_sdesc_sw128(y0 + (j >> 2) * C::YH_BYTES + (j & 3) * 2048, 8192, 1024);
-            const uint64_t bd = make_sdesc_sw128(h0 + (j >> 2) * C::HH_BYTES + (j & 3) * 32, 16, 1024);
+            const uint64_t ad = adesc0 + so + (uint64_t)(((j >> 2) * C::YH_BYTES + (j & 3) * 2048) >> 4);
+            const uint64_t bd = bdesc0 + so + (uint64_t)(((j >> 2) * C::HH_BYTES + (j & 3) * 32) >> 4);
             umma_f16(d, ad, bd, idesc, (kb | j) ? 1u : 0u);
           }
           umma_commit(&empty[st]);
+          if (kb == p.NKB - 1) umma_commit(&t_full[slot]);
         }
-        umma_commit(&t_full[slot]);
+        __syncwarp();
       }
     }
   } else if (warp == 9) {

@@ -202,24 +202,26 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     }
   } else if (warp == 4 * C::NSET) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(128, K, /*A (dY) K-major*/ 0, /*B (W) MN-major*/ 1);
-      for (int i = 0; i < n_my; ++i) {
-        const int st = i % C::NST, slot = i & 1;
-        mbar_wait(&full[st], (i / C::NST) & 1);
-        mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
-        tc_fence_after();
-        const uint32_t y0 = sbase + st * C::STAGE, w0 = y0 + C::Y_BYTES;
+    // whole warp waits, one elected lane issues; descriptors are a per-stage base + compile-time offsets (see tc_tail.cu)
+    constexpr uint32_t idesc = make_idesc_bf16(128, K, /*A (dY) K-major*/ 0, /*B (W) MN-major*/ 1);
+    const uint64_t adesc0 = make_sdesc_sw128(sbase, 16, 1024);
+    const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::Y_BYTES, G * 128, 1024);
+    for (int i = 0; i < n_my; ++i) {
+      const int st = i % C::NST, slot = i & 1;
+      mbar_wait(&full[st], (i / C::NST) & 1);
+      mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
         const uint32_t d = tmem_base + slot * K;
 #pragma unroll
-        for (int j = 0; j < G / 16; ++j) {
-          const uint64_t ad = make_sdesc_sw128(y0 + (j >> 2) * 16384 + (j & 3) * 32, 16, 1024);
-          const uint64_t bd = make_sdesc_sw128(w0 + j * 2048, G * 128, 1024);
-          umma_f16(d, ad, bd, idesc, j ? 1u : 0u);
-        }
+        for (int j = 0; j < G / 16; ++j)
+          umma_f16(d, adesc0 + so + (uint64_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4), bdesc0 + so + (uint64_t)((j * 2048) >> 4),
+                   idesc, j ? 1u : 0u);
         umma_commit(&empty[st]);
         umma_commit(&t_full[slot]);
       }
+      __syncwarp();
     }
   } else if (warp >= 4 * C::NSET + 2) {
     // ===================== auxiliary warps: idx_g -> one destination list per class =====================

@@ -144,36 +144,41 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
   } else if (warp == 4) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(128, BN, C::A_MN ? 1 : 0, C::B_MN ? 1 : 0);
-      constexpr uint32_t idesc_ones = make_idesc_bf16(128, 16, 1, 0);
-      int it = 0, n = 0;
-      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
-        const HeadItem wi = head_item(p, w);
-        if (wi.kb1 <= wi.kb0) continue;
-        const int slot = n & 1;
-        mbar_wait(&t_empty[slot], ((n >> 1) & 1) ^ 1);
+    // whole warp waits, one elected lane issues; descriptors are a per-stage base + compile-time offsets (see tc_tail.cu)
+    constexpr uint32_t idesc = make_idesc_bf16(128, BN, C::A_MN ? 1 : 0, C::B_MN ? 1 : 0);
+    constexpr uint32_t idesc_ones = make_idesc_bf16(128, 16, 1, 0);
+    const uint64_t adesc0 = C::A_MN ? make_sdesc_sw128(sbase, 8192, 1024) : make_sdesc_sw128(sbase, 16, 1024);
+    const uint64_t bdesc0 = C::B_MN ? make_sdesc_sw128(sbase + C::A_BYTES, 8192, 1024) : make_sdesc_sw128(sbase + C::A_BYTES, 16, 1024);
+    const uint64_t odesc = make_sdesc_sw128(sbase + C::OFF_ONES, 16, 1024);
+    int it = 0, n = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+      const HeadItem wi = head_item(p, w);
+      if (wi.kb1 <= wi.kb0) continue;
+      const int slot = n & 1;
+      mbar_wait(&t_empty[slot], ((n >> 1) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t dcol = tmem_base + slot * C::TS;
+      const bool with_db = MODE == HEAD_DW && p.dbias != nullptr && wi.nt == 0;
+      for (int kb = wi.kb0; kb < wi.kb1; ++kb, ++it) {
+        const int st = it % C::NST;
+        mbar_wait(&full[st], (it / C::NST) & 1);
         tc_fence_after();
-        const uint32_t dcol = tmem_base + slot * C::TS;
-        const bool with_db = MODE == HEAD_DW && p.dbias != nullptr && wi.nt == 0;
-        for (int kb = wi.kb0; kb < wi.kb1; ++kb, ++it) {
-          const int st = it % C::NST;
-          mbar_wait(&full[st], (it / C::NST) & 1);
-          tc_fence_after();
-          const uint32_t a0 = sbase + st * C::STAGE, b0 = a0 + C::A_BYTES;
+        if (elect_one()) {
+          const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
 #pragma unroll
           for (int j = 0; j < 4; ++j) {
-            const uint64_t ad = C::A_MN ? make_sdesc_sw128(a0 + j * 2048, 8192, 1024) : make_sdesc_sw128(a0 + j * 32, 16, 1024);
-            const uint64_t bd = C::B_MN ? make_sdesc_sw128(b0 + j * 2048, 8192, 1024) : make_sdesc_sw128(b0 + j * 32, 16, 1024);
+            const uint64_t ad = adesc0 + so + (uint64_t)((C::A_MN ? j * 2048 : j * 32) >> 4);
+            const uint64_t bd = bdesc0 + so + (uint64_t)((C::B_MN ? j * 2048 : j * 32) >> 4);
             const uint32_t acc = (kb > wi.kb0 || j > 0) ? 1u : 0u;
             umma_f16(dcol, ad, bd, idesc, acc);
-            if (with_db) umma_f16(dcol + BN, ad, make_sdesc_sw128(sbase + C::OFF_ONES, 16, 1024), idesc_ones, acc);
+            if (with_db) umma_f16(dcol + BN, ad, odesc, idesc_ones, acc);
           }
           umma_commit(&empty[st]);
+          if (kb == wi.kb1 - 1) umma_commit(&t_full[slot]);
         }
-        umma_commit(&t_full[slot]);
-        ++n;
+        __syncwarp();
       }
+      ++n;
     }
   } else {
     // ===================== epilogue (thread = accumulator row) =====================

@@ -3,15 +3,17 @@
 // Forward + fused BCE (PAPER.md:97 "gather-once, dense GEMM per group", :111 Eq. 3):
 //   persistent CTAs, one per SM.  A CTA owns a pair of 128-row batch tiles and a stripe of groups.
 //   per (group g, batch tile): Z[128 x G] = H_g[128 x K] * W_g^T, H_g = X[:, idx_g] gathered from X^T.
-//   warp roles (448 threads):
-//     warps 0-7   epilogue: TMEM -> registers -> sigmoid/softplus (1 MUFU per logit) -> bf16 dY
-//                 -> swizzled smem tile -> TMA store; loss partial per thread.  Two halves of 4 warps
-//                 work on alternate tiles; a thread owns ONE batch row for the whole kernel, so its
-//                 CSR target row is walked once with a running cursor.
-//     warps 8-11  gather producers: cp.async 16-B chunks of X^T rows idx_g into the swizzled H image.
-//     warp 12     MMA issuer (one thread): tcgen05.mma M=128, N=G, K=16 x (K/16) into a TMEM slot ring.
-//     warp 13     TMA loader of W_g (the [G x K] block is contiguous in W).
+//   warp roles (704 threads):
+//     warps 0-15  epilogue: TMEM -> registers -> sigmoid/softplus (1 MUFU per logit) -> bf16 dY
+//                 -> swizzled smem tile -> TMA store; loss partial per thread.  Four sets of 4 warps
+//                 work on tiles T = set mod 4 (the epilogue is a latency chain per warp: with two sets the
+//                 schedulers sat idle 42 % of the time); a thread owns ONE batch row for the whole kernel,
+//                 so its CSR target row is walked once with a running cursor.
+//     warps 16-19 gather producers: cp.async 16-B chunks of X^T rows idx_g into the swizzled H image.
+//     warp 20     MMA issuer (one thread): tcgen05.mma M=128, N=G, K=16 x (K/16) into a TMEM slot ring.
+//     warp 21     TMA loader of W_g (the [G x K] block is contiguous in W).
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -75,25 +77,27 @@ struct FwdParams {
 };
 
 template <int G, int K> struct FwdCfg {
-  static constexpr int HS = (G == 128 && K == 128) ? 3 : 4;     // H stages
-  static constexpr int LAG = 2;                                 // producer completion lag (<= HS-1)
+  static constexpr int NSET = (G == 128 && K == 128) ? 2 : 4;   // epilogue sets (4 warps each); what shared memory allows
+  static constexpr int HS = 3;                                  // H stages
+  static constexpr int LAG = 1;                                 // producer completion lag (< HS-1, or the MMAs serialise)
   static constexpr int H_BYTES = K * 256;                       // [2 m-blocks][K rows][128 B]
   static constexpr int W_BYTES = G * K * 2;                     // [K/64 k-blocks][G rows][128 B]
   static constexpr int WS = W_BYTES <= 16384 ? 3 : 2;           // W stages
-  static constexpr int ST_BYTES = 128 * (G < 64 ? G : 64) * 2;  // one dY staging tile (<= 64 labels wide) per epilogue half
+  static constexpr int ST_BYTES = 128 * (G < 64 ? G : 64) * 2;  // one dY staging tile (<= 64 labels wide) per epilogue set
   static constexpr int NSLOT = (512 / G) >= 8 ? 8 : (512 / G);  // TMEM accumulator ring (G columns each)
   static constexpr int OFF_H = 0;
   static constexpr int OFF_W = OFF_H + HS * H_BYTES;
   static constexpr int OFF_ST = OFF_W + WS * W_BYTES;
-  static constexpr int OFF_BIAS = OFF_ST + 2 * ST_BYTES;        // [8 warps][G] fp32
-  static constexpr int OFF_BAR = OFF_BIAS + 8 * G * 4;
+  static constexpr int OFF_BIAS = OFF_ST + NSET * ST_BYTES;     // [16 warps][G] fp32
+  static constexpr int OFF_BAR = OFF_BIAS + 4 * NSET * G * 4;
   static constexpr int NBAR = 2 * HS + 2 * WS + 2 * NSLOT;
   static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;           // tmem base, loss scratch
-  static constexpr int SMEM = OFF_MISC + 64 + 1024;             // + alignment slack
+  static constexpr int SMEM = OFF_MISC + 128 + 1024;            // + alignment slack
+  static constexpr int THREADS = (4 * NSET + 6) * 32;
 };
 
 template <int G, int K>
-__global__ void __launch_bounds__(448, 1)
+__global__ void __launch_bounds__(FwdCfg<G, K>::THREADS, 1)
 tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmY, const FwdParams p) {
   using C = FwdCfg<G, K>;
   extern __shared__ uint8_t smem_raw[];
@@ -105,9 +109,9 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   uint64_t* w_full = bars + 2 * C::HS;           // [WS]  count 1 + tx
   uint64_t* w_empty = w_full + C::WS;            // [WS]  count 1 (umma commit)
   uint64_t* t_full = w_empty + C::WS;            // [NSLOT] count 1 (umma commit)
-  uint64_t* t_empty = t_full + C::NSLOT;         // [NSLOT] count 4 (epilogue warps of one half)
+  uint64_t* t_empty = t_full + C::NSLOT;         // [NSLOT] count 4 (epilogue warps of one set)
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
-  float* loss_red = reinterpret_cast<float*>(smem + C::OFF_MISC + 16);   // [8]
+  float* loss_red = reinterpret_cast<float*>(smem + C::OFF_MISC + 16);   // [4 * NSET]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int pr = blockIdx.x % p.NP, stripe = blockIdx.x / p.NP;
@@ -122,16 +126,17 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     for (int i = 0; i < C::NSLOT; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
     fence_barrier_init();
   }
-  if (warp == 13 && lane == 0) { tma_prefetch_desc(&tmW); tma_prefetch_desc(&tmY); }
-  if (warp == 12) tmem_alloc<512>(tmem_slot);
+  constexpr int EW = 4 * C::NSET;                                          // epilogue warps
+  if (warp == EW + 5 && lane == 0) { tma_prefetch_desc(&tmW); tma_prefetch_desc(&tmY); }
+  if (warp == EW + 4) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  if (warp >= 8 && warp < 12) {
+  if (warp >= EW && warp < EW + 4) {
     // ===================== gather producers =====================
-    const int pw = warp - 8;
+    const int pw = warp - EW;
     constexpr int RPW = K / 4;                       // rows (slots) per producer warp
     const int sub = lane >> 4, c = lane & 15;        // two rows per instruction, 16 chunks of 16 B per row
     const uint32_t dst_lane = (uint32_t)((c >> 3) * (K * 128) + (((c & 7)) << 4));
@@ -182,32 +187,36 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         if (lane == 0) mbar_arrive(&h_full[T % C::HS]);
       }
     }
-  } else if (warp == 12) {
+  } else if (warp == EW + 4) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(128, G, /*A MN-major*/ 1, /*B K-major*/ 0);
-      for (int T = 0; T < total; ++T) {
-        const int gl = T >> tsh, which = T & tsh;
-        const int ws = gl % C::WS, hs = T % C::HS, slot = T % C::NSLOT;
-        if (which == 0) mbar_wait(&w_full[ws], (gl / C::WS) & 1);
-        mbar_wait(&h_full[hs], (T / C::HS) & 1);
-        mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
-        tc_fence_after();
-        const uint32_t a0 = sbase + C::OFF_H + hs * C::H_BYTES;
-        const uint32_t b0 = sbase + C::OFF_W + ws * C::W_BYTES;
+    // The whole warp walks the loop and waits; one elected lane issues.  (Issuing from inside `if (lane == 0)` makes
+    // ptxas wrap every tcgen05 instruction in an elect/branch loop, and rebuilding both descriptors per MMA is a
+    // chain of uniform-datapath ops: together ~1100 cycles per tile, which was this kernel's critical path.)
+    constexpr uint32_t idesc = make_idesc_bf16(128, G, /*A MN-major*/ 1, /*B K-major*/ 0);
+    const uint64_t adesc0 = make_sdesc_sw128(sbase + C::OFF_H, K * 128, 1024);
+    const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::OFF_W, 16, 1024);
+    for (int T = 0; T < total; ++T) {
+      const int gl = T >> tsh, which = T & tsh;
+      const int ws = gl % C::WS, hs = T % C::HS, slot = T % C::NSLOT;
+      if (which == 0) mbar_wait(&w_full[ws], (gl / C::WS) & 1);
+      mbar_wait(&h_full[hs], (T / C::HS) & 1);
+      mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t ad0 = adesc0 + (uint64_t)((hs * C::H_BYTES) >> 4);       // the address field never carries out
+        const uint64_t bd0 = bdesc0 + (uint64_t)((ws * C::W_BYTES) >> 4);
         const uint32_t d = tmem_base + slot * G;
 #pragma unroll
-        for (int j = 0; j < K / 16; ++j) {
-          const uint64_t ad = make_sdesc_sw128(a0 + j * 2048, K * 128, 1024);
-          const uint64_t bd = make_sdesc_sw128(b0 + (j >> 2) * (G * 128) + (j & 3) * 32, 16, 1024);
-          umma_f16(d, ad, bd, idesc, j > 0 ? 1u : 0u);
-        }
+        for (int j = 0; j < K / 16; ++j)
+          umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * (G * 128) + (j & 3) * 32) >> 4), idesc,
+                   j > 0 ? 1u : 0u);
         umma_commit(&h_empty[hs]);
         umma_commit(&t_full[slot]);
         if (which == tsh) umma_commit(&w_empty[ws]);
       }
+      __syncwarp();
     }
-  } else if (warp == 13) {
+  } else if (warp == EW + 5) {
     // ===================== W loader =====================
     if (lane == 0) {
       for (int gl = 0; gl < ngl; ++gl) {
@@ -222,9 +231,9 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     }
   } else {
     // ===================== epilogue: every warp is self-contained (own rows, own staging, own TMA stores) =====
-    const int half = warp >> 2, q = warp & 3;
+    const int set = warp >> 2, q = warp & 3;                   // set s works on tiles T = s (mod NSET)
     const int row = q * 32 + lane;                             // row of the batch tile == TMEM lane
-    const int my_bt = 2 * pr + (ntp == 2 ? half : 0);
+    const int my_bt = 2 * pr + (ntp == 2 ? (set & 1) : 0);
     const int b = my_bt * 128 + row;
     const bool valid_row = b < p.B;
     int pc = 0, pe = 0;
@@ -237,11 +246,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     const float hs = 0.5f * p.s;
     // this warp's 32 rows of the half's staging tile(s); rows are 128 B (G >= 64) or 64 B (G = 32)
     constexpr int ROWB = G >= 64 ? 128 : 64;
-    const uint32_t stage_w = sbase + C::OFF_ST + half * C::ST_BYTES + q * 32 * ROWB;
+    const uint32_t stage_w = sbase + C::OFF_ST + set * C::ST_BYTES + q * 32 * ROWB;
     const uint32_t stage_row = stage_w + lane * ROWB;
     const uint32_t swz = G >= 64 ? (uint32_t)(lane & 7) : (uint32_t)((lane >> 1) & 3);
     const uint32_t sbias_w = sbase + C::OFF_BIAS + warp * G * 4;
-    for (int T = half; T < total; T += 2) {
+    for (int T = set; T < total; T += C::NSET) {
       const int gl = T >> tsh;
       const int64_t g = stripe + (int64_t)gl * p.S;
       const int nl = (int)min((int64_t)G, p.L - g * G);
@@ -279,13 +288,12 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * G;
       float R[4] = {0.f, 0.f, 0.f, 0.f}, P[4] = {1.f, 1.f, 1.f, 1.f};
-      uint32_t v[2][32];
-      tmem_ld32(taddr, v[0]);
+      uint32_t v[32];                 // one chunk at a time: 16 epilogue warps hide the TMEM latency, registers are short
 #pragma unroll
       for (int sc = 0; sc < G / 32; ++sc) {
+        tmem_ld32(taddr + sc * 32, v);
         tmem_ld_wait();
-        if (sc + 1 < G / 32) tmem_ld32(taddr + (sc + 1) * 32, v[(sc + 1) & 1]);
-        else {
+        if (sc + 1 == G / 32) {
           // all of this warp's TMEM reads are done: hand the accumulator slot back to the MMA issuer
           tc_fence_before();
           __syncwarp();
@@ -296,11 +304,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         const int nvalid = nl - sc * 32;
         const uint32_t sb = sbias_w + sc * 128;
         if (slow) {
-          if (p.bias) epi32<true, true>(v[sc & 1], sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
-          else epi32<true, false>(v[sc & 1], sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+          if (p.bias) epi32<true, true>(v, sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+          else epi32<true, false>(v, sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
         } else {
-          if (p.bias) epi32<false, true>(v[sc & 1], sb, 0u, 32, p.s, hs, R, P, out, nullptr);
-          else epi32<false, false>(v[sc & 1], sb, 0u, 32, p.s, hs, R, P, out, nullptr);
+          if (p.bias) epi32<false, true>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
+          else epi32<false, false>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
         }
         if (sc & 1) {   // 64 factors in [1/2,1) at most per product: fold into the loss, restart the chains
           loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
@@ -321,7 +329,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) {
-              tma_store_3d(&tmY, smem + C::OFF_ST + half * C::ST_BYTES + q * 32 * ROWB, (sc >> 1) * 64, my_bt * 128 + q * 32, (int)g);
+              tma_store_3d(&tmY, smem + C::OFF_ST + set * C::ST_BYTES + q * 32 * ROWB, (sc >> 1) * 64, my_bt * 128 + q * 32, (int)g);
               bulk_commit();
             }
           }
@@ -339,11 +347,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 12) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
+  if (warp == EW + 4) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
   if (threadIdx.x == 0 && p.partials) {
     float t = 0.f;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) t += loss_red[i];
+    for (int i = 0; i < EW; ++i) t += loss_red[i];
     p.partials[blockIdx.x] = t;
   }
 }
@@ -408,7 +416,7 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   if (partials && grid < s->n_partials)   // partials beyond the grid stay zero from create / earlier calls: clear them
     HASTE_CUDA_TRY(cudaMemsetAsync(partials + grid, 0, (size_t)(s->n_partials - grid) * sizeof(float), st));
   HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-  tc_fwd_kernel<G, K><<<grid, 448, C::SMEM, st>>>(tmW, tmY, p);
+  tc_fwd_kernel<G, K><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }

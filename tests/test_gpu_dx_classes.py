@@ -1,0 +1,127 @@
+"""-m gpu parity of the on-chip accumulating dX kernel (csrc/tc_dx_acc.cu) on the cases its design turns on:
+features of all three destination classes (TMEM columns / shared-memory rows / L2 reductions), slot ranges that
+start and end exactly at the class boundaries, groups whose idx row is NOT strictly increasing (duplicates,
+unsorted: reading R4, they take the atomic path) mixed with strictly increasing ones, ragged batch tiles, and
+both fan-ins the kernel is built for.  dX = sum_g dY_g W_g scattered by idx_g.
+
+Two gates per case, both through haste_dy_pack so that only the backward is under test:
+  * small-integer dY and W: dX (and dW, db) must equal the fp64 oracle EXACTLY, whatever the order of additions;
+  * real-valued dY rounded to bf16: rel-L2 <= 1e-4 against the oracle run on the same rounded dY.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_01117_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _boundary_idx(rng, NG, K, d, kind):
+    """idx rows [NG,K] int32 in [0,d) that stress the class boundaries of tc_dx_acc.cu (255/383 TMEM features for
+    K = 128/64, then as many shared-memory rows as fit, then L2)."""
+    tf = 512 - 2 * K - 1
+    idx = np.empty((NG, K), dtype=np.int32)
+    for g in range(NG):
+        mode = g % 6 if kind == "mixed" else 0
+        if mode == 0:      # strictly increasing, uniform over [0,d)
+            row = np.sort(rng.choice(d, size=K, replace=False))
+        elif mode == 1:    # a run of consecutive features straddling the TMEM / shared-memory boundary
+            lo = max(0, min(d - K, tf - K // 2))
+            row = np.arange(lo, lo + K)
+        elif mode == 2:    # everything at the top of the feature range (L2 class when d is large), strictly increasing
+            row = np.arange(d - K, d)
+        elif mode == 3:    # duplicates inside the row (sorted, NOT strict): atomic path
+            row = np.sort(rng.choice(d, size=K, replace=True))
+            row[K // 2] = row[K // 2 - 1]
+        elif mode == 4:    # unsorted, distinct
+            row = rng.permutation(d)[:K]
+            if np.all(np.diff(row) > 0):
+                row = row[::-1]
+        else:              # everything below the first boundary (one class owns the whole row)
+            row = np.sort(rng.choice(min(d, max(K, tf // 2)), size=K, replace=False))
+        idx[g] = row
+    return idx
+
+
+CASES = [
+    # B, d, NG (L = G*NG - 5), G, K, kind
+    (300, 768, 23, 64, 128, "mixed"),     # config-3 tile shape: 255 TMEM + ~295 smem + L2 features, ragged batch tile
+    (128, 1024, 17, 64, 64, "mixed"),     # config-4 tile shape: 383 TMEM features, d = 1024
+    (130, 768, 9, 128, 128, "mixed"),     # wide groups: two operand stages, fewer shared-memory rows
+    (64, 400, 11, 128, 64, "mixed"),      # d barely above the TMEM class (383 features): 17 shared-memory rows, no L2 class
+    (257, 768, 40, 64, 128, "strict"),    # every row strictly increasing (the fast path only)
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=lambda c: "B%d_d%d_NG%d_G%d_K%d_%s" % c)
+def test_dx_classes_exact_and_close(oracle, case):
+    from paper_2606_01117_b200 import haste
+    from gpu_util import TailRun, dy_rounded
+    B, d, NG, G, K, kind = case
+    L = G * NG - 5
+    inp = synth.small_case(100 + B + d, B, d, L, G, K, dtype="bf16", with_bias=False, w_std=0.05)
+    rng = np.random.RandomState(B + d + K)
+    inp.idx = _boundary_idx(rng, NG, K, d, kind)
+    flags = haste.HASTE_IDX_SORTED_DISTINCT if kind == "strict" else 0
+
+    # ---- gate 1: integers, exact
+    Wi = rng.randint(-4, 5, size=(L, K)).astype(np.float32)
+    Xi = rng.randint(-4, 5, size=(B, d)).astype(np.float32)
+    dYi = rng.randint(-3, 4, size=(B, L)).astype(np.float32)
+    inp.X, inp.W = Xi, Wi
+    inp.bits["X"], inp.bits["W"] = synth.round_bf16(Xi)[0].reshape(B, d), synth.round_bf16(Wi)[0].reshape(L, K)
+    run = TailRun(inp, G, flags=flags, dw_dtype="f32")
+    assert run.layer.kernel_family == 1
+    out = run.backward(dY_BL=dYi)
+    ref = oracle.tail_backward(inp.X, inp.idx, inp.W, dYi.astype(np.float64), G)
+    assert np.array_equal(out["dX"].astype(np.float64), ref["dX"])
+    assert np.array_equal(out["dW"].astype(np.float64), ref["dW"])
+    assert np.array_equal(out["db"].astype(np.float64), ref["db"])
+    # a second call on the same handle must give the same answer (accumulators are re-zeroed per call)
+    out2 = run.backward(dY_BL=dYi)
+    assert np.array_equal(out2["dX"], out["dX"])
+
+    # ---- gate 2: real values, accumulation error only
+    Wr = (rng.standard_normal((L, K)) * 0.05).astype(np.float32)
+    dYr = (rng.standard_normal((B, L)) / B).astype(np.float32)
+    bits, Wr = synth.round_bf16(Wr)
+    inp.W, inp.bits["W"] = Wr.reshape(L, K), bits.reshape(L, K)
+    run = TailRun(inp, G, flags=flags, dw_dtype="f32")
+    dYq = dy_rounded(inp, dYr)
+    out = run.backward(dY_BL=dYq)
+    ref = oracle.tail_backward(inp.X, inp.idx, inp.W, dYq.astype(np.float64), G)
+    for k in ("dX", "dW", "db"):
+        err = oracle.rel_l2(out[k], ref[k])
+        assert err <= 1e-4, (k, err)
+    # per-class slices of dX on their own (a class that silently dropped its adds would hide in the global norm)
+    tf = 512 - 2 * K - 1
+    for lo, hi in ((0, min(d, tf)), (min(d, tf), min(d, tf + 120)), (max(0, d - 100), d)):
+        if hi > lo and np.linalg.norm(ref["dX"][:, lo:hi]) > 0:
+            assert oracle.rel_l2(out["dX"][:, lo:hi], ref["dX"][:, lo:hi]) <= 1e-4, (lo, hi)
+
+
+def test_dx_red_kernel_still_matches():
+    """The first-version kernel (L2 reductions only, HASTE_DX_KERNEL=red) is kept as a comparison point: same answer."""
+    import subprocess, sys, os, textwrap
+    code = textwrap.dedent("""
+        import numpy as np, sys
+        sys.path.insert(0, %r); sys.path.insert(0, %r)
+        from paper_2606_01117_b200 import synth
+        import oracle
+        from gpu_util import TailRun
+        B, d, L, G, K = 200, 768, 64 * 9 + 3, 64, 128
+        inp = synth.small_case(77, B, d, L, G, K, dtype="bf16", with_bias=False, w_std=0.05)
+        rng = np.random.RandomState(5)
+        dYi = rng.randint(-3, 4, size=(B, L)).astype(np.float32)
+        Wi = rng.randint(-4, 5, size=(L, K)).astype(np.float32)
+        inp.W = Wi; inp.bits["W"] = synth.round_bf16(Wi)[0].reshape(L, K)
+        run = TailRun(inp, G, dw_dtype="f32")
+        out = run.backward(dY_BL=dYi)
+        ref = oracle.tail_backward(inp.X, inp.idx, inp.W, dYi.astype(np.float64), G)
+        err = oracle.rel_l2(out["dX"], ref["dX"])
+        assert err <= 1e-6, err
+        print("ok")
+    """) % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, HASTE_DX_KERNEL="red")
+    r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "ok" in r.stdout, r.stderr[-2000:]
