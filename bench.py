@@ -56,14 +56,44 @@ def _peaks():
 
 
 class ClockSampler:
+    """SM clock, power and throttle reasons sampled DURING the timed region: an NVML polling thread (a sample every
+    ~2 ms, so that even a 20-step region of ~16 ms is covered), `nvidia-smi -lms` as the fallback."""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    BITS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
     def __init__(self, index):
         self.index = index
         self.proc = None
         self.f = None
+        self.thread = None
+        self.stop_flag = False
+        self.rows = []      # (sm_mhz, max_mhz, watts, reason_mask)
+
+    def _nvml_loop(self, nv, h):
+        reasons_fn = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or getattr(nv, "nvmlDeviceGetCurrentClocksThrottleReasons")
+        smax = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+        while not self.stop_flag:
+            try:
+                self.rows.append((nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM), smax, nv.nvmlDeviceGetPowerUsage(h) / 1000.0, int(reasons_fn(h))))
+            except Exception:
+                pass
+            time.sleep(0.002)
 
     def start(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            # NVML enumerates physical devices: map through CUDA_VISIBLE_DEVICES when it is a plain index list
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            phys = self.index
+            if vis and all(t.strip().isdigit() for t in vis.split(",")):
+                phys = int(vis.split(",")[self.index])
+            h = nv.nvmlDeviceGetHandleByIndex(phys)
+            self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.thread = None
         try:
             self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
@@ -73,6 +103,17 @@ class ClockSampler:
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.thread is not None:
+            self.stop_flag = True
+            self.thread.join(timeout=2)
+            if self.rows:
+                mask = 0
+                for r in self.rows:
+                    mask |= r[3]
+                out = {"sm_mhz": float(np.median([r[0] for r in self.rows])), "sm_max_mhz": float(max(r[1] for r in self.rows)),
+                       "power_w_max": float(max(r[2] for r in self.rows)), "samples": len(self.rows),
+                       "reasons": sorted(n for b, n in self.BITS.items() if mask & b), "source": "nvml"}
+            return out
         if not self.proc:
             return out
         time.sleep(0.06)
@@ -100,7 +141,7 @@ class ClockSampler:
         os.unlink(self.f.name)
         if sm:
             out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
-                   "samples": len(sm), "reasons": sorted(reasons)}
+                   "samples": len(sm), "reasons": sorted(reasons), "source": "nvidia-smi"}
         return out
 
 
@@ -171,7 +212,7 @@ def run_reference(args, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="haste", choices=["haste", "reference"])
     ap.add_argument("--workload", default=WORKLOAD, help="synth.CONFIGS key (default: the 670K-label config the metric is quoted on)")
@@ -279,9 +320,10 @@ def main():
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
-    layer.set_profiling(args.steps)
+    nprof = min(args.steps, 1024)      # per-kernel event ring of the library: the last nprof calls of the timed region
+    layer.set_profiling(nprof)
     if use_head:
-        head.set_profiling(args.steps)
+        head.set_profiling(nprof)
     launches[0] = 0
     sampler = ClockSampler(local)
     if rank == 0:
@@ -292,10 +334,10 @@ def main():
     # per-kernel device times of the timed region (CUDA events recorded inside the library, on the launch stream)
     kn = {"forward": haste.KERNEL_FORWARD, "dW": haste.KERNEL_DW, "dX": haste.KERNEL_DX,
           "prep_fwd": haste.KERNEL_PREP_FWD, "prep_bwd": haste.KERNEL_PREP_BWD, "post_bwd": haste.KERNEL_POST_BWD}
-    kms = {k: [layer.kernel_ms(v, a) for a in range(args.steps)] for k, v in kn.items()}
+    kms = {k: [layer.kernel_ms(v, a) for a in range(nprof)] for k, v in kn.items()}
     if use_head:
-        kms["head_forward"] = [head.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(args.steps)]
-        kms["head_backward"] = [head.kernel_ms(haste.KERNEL_DW, a) for a in range(args.steps)]
+        kms["head_forward"] = [head.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nprof)]
+        kms["head_backward"] = [head.kernel_ms(haste.KERNEL_DW, a) for a in range(nprof)]
     layer.set_profiling(0)
     if use_head:
         head.set_profiling(0)

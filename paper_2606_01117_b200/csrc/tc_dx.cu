@@ -189,7 +189,8 @@ int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const vo
     return use_red ? launch_dx_red<G_, K_>(s, sh, idx, W, dY, dXt, st) : tc_tail_dx_acc(s, sh, idx, W, dY, dXt, st)
   HASTE_DX(64, 128); HASTE_DX(64, 64); HASTE_DX(128, 64); HASTE_DX(128, 128);
 #undef HASTE_DX
-  return HASTE_ERR_UNSUPPORTED;   // G = 32: the caller runs the CUDA-core kernel
+  if (sh.G == 32 && (sh.K == 64 || sh.K == 128)) return tc_tail_dx_acc(s, sh, idx, W, dY, dXt, st);   // 64-byte-swizzle operand: acc kernel only
+  return HASTE_ERR_UNSUPPORTED;
 }
 
 }  // namespace haste

@@ -45,7 +45,7 @@ struct DxAccParams {
 template <int G, int K, int NST_> struct DxAccCfg {
   static constexpr int NSET = 4;                              // epilogue sets: 0 = TA, 1 = SB, 2 = TC, 3 = SD
   static constexpr int NLIST = NSET + 1;                      // + the L list
-  static constexpr int Y_BYTES = G * 256;                     // [G/64 k-blocks][128 batch rows][128 B]
+  static constexpr int Y_BYTES = G * 256;                     // [G/64 k-blocks][128 batch rows][128 B]; G = 32: [128 rows][64 B]
   static constexpr int W_BYTES = G * K * 2;                   // [K/64 slot atoms][G label rows][128 B]
   static constexpr int STAGE = Y_BYTES + W_BYTES;
   static constexpr int NST = NST_;                            // operand stages (dY tile + W_g) in flight
@@ -195,7 +195,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         mbar_arrive_expect_tx(&full[st], C::STAGE);
         uint8_t* s0 = smem + st * C::STAGE;
 #pragma unroll
-        for (int kb = 0; kb < G / 64; ++kb) tma_load_3d(s0 + kb * 16384, &tmY, &full[st], kb * 64, bt * 128, (int)g);
+        for (int kb = 0; kb < (G >= 64 ? G / 64 : 1); ++kb) tma_load_3d(s0 + kb * 16384, &tmY, &full[st], kb * 64, bt * 128, (int)g);
 #pragma unroll
         for (int a = 0; a < K / 64; ++a) tma_load_2d(s0 + C::Y_BYTES + a * (G * 128), &tmW, &full[st], a * 64, (int)(g * G));
       }
@@ -204,7 +204,8 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     // ===================== MMA issuer =====================
     // whole warp waits, one elected lane issues; descriptors are a per-stage base + compile-time offsets (see tc_tail.cu)
     constexpr uint32_t idesc = make_idesc_bf16(128, K, /*A (dY) K-major*/ 0, /*B (W) MN-major*/ 1);
-    const uint64_t adesc0 = make_sdesc_sw128(sbase, 16, 1024);
+    // A = the dY tile, K-major: 128-byte rows (64 labels per k-block) or, for G = 32, 64-byte rows with the 64-byte swizzle
+    const uint64_t adesc0 = G >= 64 ? make_sdesc_sw128(sbase, 16, 1024) : make_sdesc_sw64(sbase, 16, 512);
     const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::Y_BYTES, G * 128, 1024);
     for (int i = 0; i < n_my; ++i) {
       const int st = i % C::NST, slot = i & 1;
@@ -400,8 +401,8 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   {
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
     const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
-    const uint32_t box[3] = {64, 128, 1};
-    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, 128);
+    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 128, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
     if (rc) return rc;
   }
   {
@@ -441,6 +442,7 @@ int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, cons
     return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, st);                                       \
   }
   HASTE_DXA(64, 128, 3); HASTE_DXA(64, 64, 3); HASTE_DXA(128, 64, 3); HASTE_DXA(128, 128, 2);
+  HASTE_DXA(32, 64, 3); HASTE_DXA(32, 128, 3);
 #undef HASTE_DXA
   return HASTE_ERR_UNSUPPORTED;
 }

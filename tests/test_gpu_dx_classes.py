@@ -50,6 +50,8 @@ CASES = [
     (130, 768, 9, 128, 128, "mixed"),     # wide groups: two operand stages, fewer shared-memory rows
     (64, 400, 11, 128, 64, "mixed"),      # d barely above the TMEM class (383 features): 17 shared-memory rows, no L2 class
     (257, 768, 40, 64, 128, "strict"),    # every row strictly increasing (the fast path only)
+    (200, 768, 21, 32, 64, "mixed"),      # config-2 tile shape: G = 32 (dY tile is a 64-byte-swizzle operand)
+    (130, 768, 13, 32, 128, "mixed"),
 ]
 
 
