@@ -32,13 +32,20 @@ struct DwParams {
 };
 
 template <int G, int K, bool F32> struct DwCfg {
-  static constexpr int NE = G == 128 ? 16 : 8;              // rows of ones appended to the H image
-  static constexpr int N = K + NE;                          // MMA N
+  // G = 32: two consecutive groups form one virtual group of GV = 64 labels and KV = 2K slots (their idx rows are
+  // adjacent in memory, so are their labels).  D [64 x 2K] then holds dW_g in rows 0-31 x columns [0,K) and dW_{g+1}
+  // in rows 32-63 x columns [K,2K); the off-diagonal blocks are computed and ignored (the tensor pipe has the room).
+  static constexpr bool PAIR = G == 32;
+  static constexpr int GV = PAIR ? 64 : G;                  // MMA M
+  static constexpr int KV = PAIR ? 2 * K : K;               // gathered slots per (virtual) group
+  static constexpr int NE = GV == 128 ? 16 : 8;             // rows of ones appended to the H image
+  static constexpr int N = KV + NE;                         // MMA N
+  static_assert(N <= 256, "MMA N");
   // a k-block is 128 batch rows = two 64-row halves (one 128-byte swizzle row holds 64 bf16): the issuing thread
   // pays one barrier wait and one commit per 8 MMAs (with 64-row k-blocks its ~0.3 us loop overhead per k-block
   // was the kernel's bottleneck)
-  static constexpr int HH_BYTES = (K + 16) * 128;           // one half of the H image, multiple of 1024
-  static constexpr int YH_BYTES = G * 128;                  // one half of the dY image: [G/64 atoms][64 rows][128 B]
+  static constexpr int HH_BYTES = (KV + 16) * 128;          // one half of the H image, multiple of 1024
+  static constexpr int YH_BYTES = GV * 128;                 // one half of the dY image: [G/64 atoms][64 rows][128 B]; PAIR: [2 groups][64 rows][64 B]
   static constexpr int H_BYTES = 2 * HH_BYTES;
   static constexpr int Y_BYTES = 2 * YH_BYTES;
   static constexpr int STAGE = H_BYTES + Y_BYTES;
@@ -52,7 +59,7 @@ template <int G, int K, bool F32> struct DwCfg {
   static constexpr int NBAR = 2 * NST + 4;
   static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;
   static constexpr int SMEM = OFF_MISC + 64 + 1024;
-  static constexpr int RW = G == 128 ? 32 : 16;             // label rows per epilogue warp (M = 64 fills lanes 0-15 of a quadrant)
+  static constexpr int RW = GV == 128 ? 32 : 16;            // label rows per epilogue warp (M = 64 fills lanes 0-15 of a quadrant)
   static constexpr int NBOX = F32 ? K / 32 : K / 64;        // 128-byte output boxes per dW row
   static_assert(NST > LAG, "ring too short");
 };
@@ -82,7 +89,8 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_my = p.NG > blockIdx.x ? (int)((p.NG - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;   // groups of this CTA
+  const int64_t NGV = C::PAIR ? (p.NG + 1) / 2 : p.NG;                                               // (virtual) groups
+  const int n_my = NGV > blockIdx.x ? (int)((NGV - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;     // groups of this CTA
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], 5); mbar_init(&empty[i], 1); }
@@ -92,7 +100,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   // rows K .. K+15 of every stage's H image: bf16 1.0 (swizzling permutes equal chunks: write linearly)
   for (int e = threadIdx.x; e < C::NST * 2 * 16 * 8; e += blockDim.x) {
     const int st = e / 256, hf = (e >> 7) & 1, r = e % 128;
-    sts128(sbase + st * C::STAGE + hf * C::HH_BYTES + K * 128 + r * 16, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
+    sts128(sbase + st * C::STAGE + hf * C::HH_BYTES + C::KV * 128 + r * 16, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
   }
   fence_proxy_async_smem();
   if (warp == 9 && lane == 0) { tma_prefetch_desc(&tmY); tma_prefetch_desc(&tmO); }
@@ -105,16 +113,22 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   if (warp >= 4 && warp < 8) {
     // ===================== gather producers =====================
     const int pw = warp - 4;
-    constexpr int RPW = K / 4;                       // slots per producer warp
+    constexpr int RPW = C::KV / 4;                   // slots per producer warp
     const int sub = lane >> 3, c = lane & 7;         // 4 rows per instruction, 8 chunks of 16 B per row
-    const int32_t* idx_ptr = p.idx + pw * RPW + lane;
+    // slot (pw*RPW + lane) of virtual group v is idx[v*KV + slot]; the second half of an unpaired last virtual group
+    // (no group 2v+1) re-reads the first half's indices: its dY is zero-filled, its output rows are clipped
+    auto idx_of = [&](int64_t v) -> int {
+      int64_t off = v * C::KV + pw * RPW + lane;
+      if (C::PAIR && pw * RPW + lane >= K && 2 * v + 1 >= p.NG) off -= K;
+      return __ldg(p.idx + off);
+    };
     int idx_cur = 0, idx_nxt = 0;
-    if (lane < RPW && n_my > 0) idx_nxt = __ldg(idx_ptr + (int64_t)blockIdx.x * K);
+    if (lane < RPW && n_my > 0) idx_nxt = idx_of(blockIdx.x);
     int it = 0;
     for (int i = 0; i < n_my; ++i) {
       const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
       idx_cur = idx_nxt;
-      if (lane < RPW && i + 1 < n_my) idx_nxt = __ldg(idx_ptr + (g + gridDim.x) * K);
+      if (lane < RPW && i + 1 < n_my) idx_nxt = idx_of(g + gridDim.x);
       for (int kb = 0; kb < p.NKB; ++kb, ++it) {
         const int st = it % C::NST;
         mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
@@ -152,9 +166,10 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   } else if (warp == 8) {
     // ===================== MMA issuer =====================
     // whole warp waits, one elected lane issues; descriptors are a per-stage base + compile-time offsets (see tc_tail.cu)
-    constexpr uint32_t idesc = make_idesc_bf16(G, C::N, /*A (dY) MN-major*/ 1, /*B (H^T) K-major*/ 0);
+    constexpr uint32_t idesc = make_idesc_bf16(C::GV, C::N, /*A (dY) MN-major*/ 1, /*B (H^T) K-major*/ 0);
     const uint64_t bdesc0 = make_sdesc_sw128(sbase, 16, 1024);
-    const uint64_t adesc0 = make_sdesc_sw128(sbase + C::H_BYTES, 8192, 1024);
+    // A = the dY k-block as stored, MN-major: atoms of 64 labels x 128 B rows, or (PAIR) two groups of 32 labels x 64 B rows
+    const uint64_t adesc0 = C::PAIR ? make_sdesc_sw64(sbase + C::H_BYTES, 4096, 512) : make_sdesc_sw128(sbase + C::H_BYTES, 8192, 1024);
     int it = 0;
     for (int i = 0; i < n_my; ++i) {
       const int slot = i & 1;
@@ -169,7 +184,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
-            const uint64_t ad = adesc0 + so + (uint64_t)(((j >> 2) * C::YH_BYTES + (j & 3) * 2048) >> 4);
+            const uint64_t ad = adesc0 + so + (uint64_t)(((j >> 2) * C::YH_BYTES + (j & 3) * (C::PAIR ? 1024 : 2048)) >> 4);
             const uint64_t bd = bdesc0 + so + (uint64_t)(((j >> 2) * C::HH_BYTES + (j & 3) * 32) >> 4);
             umma_f16(d, ad, bd, idesc, (kb | j) ? 1u : 0u);
           }
@@ -192,9 +207,11 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
 #pragma unroll
           for (int hf = 0; hf < 2; ++hf)
 #pragma unroll
-            for (int a = 0; a < G / 64; ++a)
-              tma_load_3d(smem + st * C::STAGE + C::H_BYTES + hf * C::YH_BYTES + a * 8192, &tmY, &full[st], a * 64,
-                          kb * 128 + hf * 64, (int)g);
+            for (int a = 0; a < C::GV / 64 + (C::PAIR ? 1 : 0); ++a) {
+              uint8_t* dst = smem + st * C::STAGE + C::H_BYTES + hf * C::YH_BYTES + a * (C::PAIR ? 4096 : 8192);
+              if (C::PAIR) tma_load_3d(dst, &tmY, &full[st], 0, kb * 128 + hf * 64, (int)(2 * g + a));   // group 2v+a (zero-filled past NG)
+              else tma_load_3d(dst, &tmY, &full[st], a * 64, kb * 128 + hf * 64, (int)g);
+            }
         }
       }
     }
@@ -210,17 +227,18 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
       mbar_wait(&t_full[slot], (i >> 1) & 1);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * C::TS;
+      const uint32_t tcol = taddr + (C::PAIR && q >= 2 ? K : 0);   // PAIR: quadrants 2, 3 hold group 2v+1, whose dW sits in columns [K, 2K)
       if (p.write_dw) {
 #pragma unroll 1
         for (int c = 0; c < C::NBOX; ++c, ++nstore) {
           uint32_t out[32];
           if (F32) {
-            tmem_ld32(taddr + c * 32, out);
+            tmem_ld32(tcol + c * 32, out);
             tmem_ld_wait();
           } else {
             uint32_t v0[32], v1[32];
-            tmem_ld32(taddr + c * 64, v0);
-            tmem_ld32(taddr + c * 64 + 32, v1);
+            tmem_ld32(tcol + c * 64, v0);
+            tmem_ld32(tcol + c * 64 + 32, v1);
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
@@ -237,15 +255,15 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 4096, c * (F32 ? 32 : 64), (int)(g * G + q * C::RW));
+            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 4096, c * (F32 ? 32 : 64), (int)(g * C::GV + q * C::RW));
             bulk_commit();
           }
         }
       }
       if (p.dbias) {
-        const uint32_t v = tmem_ld1(taddr + K);
+        const uint32_t v = tmem_ld1(taddr + C::KV);
         tmem_ld_wait();
-        const int64_t l = g * G + q * C::RW + lane;
+        const int64_t l = g * C::GV + q * C::RW + lane;
         if (lane < C::RW && l < p.L) p.dbias[l] = __uint_as_float(v);
       }
       tc_fence_before();
@@ -269,8 +287,8 @@ static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const 
   {
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
     const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
-    const uint32_t box[3] = {64, 64, 1};
-    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, 128);
+    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 64, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
     if (rc) return rc;
   }
   if (dW) {
@@ -286,7 +304,7 @@ static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const 
   DwParams p;
   p.Xt = (const bf16*)Xt; p.idx = idx; p.dbias = dbias; p.write_dw = dW ? 1 : 0;
   p.B = sh.B; p.Bpad = sh.Bpad; p.NKB = ceil_div(sh.B, 128); p.L = sh.L; p.NG = sh.NG;
-  const int grid = (int)std::min<int64_t>(sh.NG, s->num_sms);
+  const int grid = (int)std::min<int64_t>(C::PAIR ? (sh.NG + 1) / 2 : sh.NG, s->num_sms);
   HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dw_kernel<G, K, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
   tc_dw_kernel<G, K, F32><<<grid, 320, C::SMEM, st>>>(tmY, tmO, p);
   HASTE_LAUNCH_CHECK();
@@ -301,9 +319,9 @@ int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_
   if (sh.G == G_ && sh.K == K_)                                                              \
     return f32 ? launch_dw<G_, K_, true>(s, sh, Xt, idx, dY, dW, dbias, st)                  \
                : launch_dw<G_, K_, false>(s, sh, Xt, idx, dY, dW, dbias, st)
-  HASTE_DW(64, 128); HASTE_DW(64, 64); HASTE_DW(128, 64); HASTE_DW(128, 128);
+  HASTE_DW(64, 128); HASTE_DW(64, 64); HASTE_DW(128, 64); HASTE_DW(128, 128); HASTE_DW(32, 64);
 #undef HASTE_DW
-  return HASTE_ERR_UNSUPPORTED;   // G = 32: the caller runs the CUDA-core kernel
+  return HASTE_ERR_UNSUPPORTED;   // G = 32 with K = 128 (the paired MMA would need N = 264): the caller runs the CUDA-core kernel
 }
 
 }  // namespace haste

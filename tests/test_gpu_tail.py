@@ -69,6 +69,7 @@ SMALL = [
     (9, 24, 40, 8, 24, "f32", True, False),           # K = d: dense layer
     (64, 128, 64 * 5 + 11, 64, 64, "bf16", True, True),
     (130, 256, 32 * 9 + 7, 32, 64, "bf16", True, False),
+    (200, 300, 32 * 8 + 5, 32, 64, "bf16", True, True),      # odd number of groups: the paired dW kernel has an unpaired last group
     (256, 256, 128 * 3 + 5, 128, 128, "bf16", True, True),
     (512, 768, 64 * 40 + 11, 64, 128, "bf16", True, True),   # config-3 tile shape, several tiles, ragged tail
     (100, 200, 64 * 3 + 1, 64, 24, "bf16", False, True),     # shape outside the tensor-core family
