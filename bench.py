@@ -215,6 +215,77 @@ def run_reference(args, cfg):
     }))
 
 
+def run_sweep(args):
+    """--sweep: BASELINE.json config 5 (kernel sweep at fixed nnz): B in {64,256,1024}, d=768, L=670091, K=64,
+    G in {1,8,16,32,64,128} (G=1 = ungrouped per-label fixed fan-in, the comparison kernel), uniform sorted idx, no head,
+    against the FLOPs-matched dense bottleneck d -> r=64 -> L in bf16 (cuBLAS through torch.matmul: comparison point,
+    not product).  Timing only (parity for config 5 lives in tests/test_gpu_configs.py); inputs are drawn on the
+    device with torch's generator (seed 1005).  One JSON line per point on stdout."""
+    import torch
+    from paper_2606_01117_b200 import haste
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peaks = _peaks()
+    d, L, K, r = 768, 670091, 64, 64
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(1005)
+    W = (torch.randn(L, K, device=dev, generator=gen) * 0.02).to(torch.bfloat16)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > L2: written between timed iterations
+    Bs = [int(x) for x in args.sweep_B.split(",")]
+    Gs = [int(x) for x in args.sweep_G.split(",")]
+    steps = min(args.steps, 10)
+    for B in Bs:
+        X = torch.randn(B, d, device=dev, generator=gen).to(torch.bfloat16)
+        rowptr = torch.arange(0, 5 * (B + 1), 5, dtype=torch.int32, device=dev)
+        col = torch.sort(torch.randint(0, L, (B, 5), device=dev, generator=gen, dtype=torch.int32), dim=1).values.reshape(-1).contiguous()
+        # dense bottleneck d -> r -> L: H = X P^T [B,r]; Z = H W^T [B,L]; backward dW = dZ^T H, dH = dZ W  (same FLOPs and W/output bytes)
+        P = (torch.randn(r, d, device=dev, generator=gen) * 0.02).to(torch.bfloat16)
+        Hh = X @ P.t()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        tb = {"fwd": [], "dW": [], "dX": []}
+        Z = torch.empty(B, L, dtype=torch.bfloat16, device=dev)
+        for it in range(steps + 2):
+            flush.fill_(it & 1)
+            ev[0].record(); torch.matmul(Hh, W.t(), out=Z); ev[1].record()
+            dWd = Z.t() @ Hh; ev[2].record()
+            dH = Z @ W; ev[3].record()
+            torch.cuda.synchronize()
+            if it >= 2:
+                tb["fwd"].append(ev[0].elapsed_time(ev[1])); tb["dW"].append(ev[1].elapsed_time(ev[2])); tb["dX"].append(ev[2].elapsed_time(ev[3]))
+        del Z, dWd, dH
+        dense = {k: float(np.median(v)) for k, v in tb.items()}
+        for G in Gs:
+            NG = -(-L // G)
+            idx = torch.empty(NG, K, dtype=torch.int32, device=dev)
+            for a in range(0, NG, 65536):       # K distinct features per group, uniform, sorted
+                b = min(NG, a + 65536)
+                idx[a:b] = torch.sort(torch.rand(b - a, d, device=dev, generator=gen).topk(K, dim=1).indices, dim=1).values.to(torch.int32)
+            layer = haste.HasteLayer(d, L, G, K, B, "bf16", flags=haste.HASTE_IDX_SORTED_DISTINCT)
+            dY = layer.alloc_dy(B)
+            dW = torch.empty(L, K, dtype=torch.bfloat16, device=dev)
+            dX = torch.empty(B, d, device=dev)
+            loss = torch.zeros(1, device=dev)
+            layer.set_profiling(1)
+            t = {"fwd": [], "dW": [], "dX": []}
+            for it in range(steps + 2):
+                flush.fill_(it & 1)
+                layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss, dY=dY)
+                layer.backward(B, X, idx, W, dY, dW=dW, dbias=None, dX=dX)
+                torch.cuda.synchronize()
+                if it >= 2:
+                    t["fwd"].append(layer.kernel_ms(haste.KERNEL_FORWARD)); t["dW"].append(layer.kernel_ms(haste.KERNEL_DW)); t["dX"].append(layer.kernel_ms(haste.KERNEL_DX))
+            Wb, ib, dYb, Xb = L * K * 2, NG * K * 4, NG * G * B * 2, B * d * 2
+            ab = {"fwd": Wb + ib + Xb + dYb, "dW": dYb + ib + Xb + Wb, "dX": dYb + Wb + ib + B * d * 4}
+            out = {"sweep": "config5", "B": B, "G": G, "K": K, "d": d, "L": L, "kernel_family": layer.kernel_family, "flush": "256 MiB fill between iterations"}
+            for k in t:
+                ms = float(np.median(t[k]))
+                out[k] = {"ms": ms, "GB/s": ab[k] / ms / 1e6, "frac_hbm": ab[k] / ms / 1e6 / peaks["hbm"], "TFLOP/s": 2.0 * B * L * K / ms / 1e9,
+                          "dense_bottleneck_ms": dense[k], "vs_dense": dense[k] / ms}
+            print(json.dumps(out), flush=True)
+            del layer, dY, dW, dX, idx
+            torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -224,9 +295,15 @@ def main():
     ap.add_argument("--workload", default=WORKLOAD, help="synth.CONFIGS key (default: the 670K-label config the metric is quoted on)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-head", action="store_true", help="time the sparse tail alone")
+    ap.add_argument("--sweep", action="store_true", help="config 5: kernel sweep over B and G at K=64 against the dense bottleneck (one JSON line per point)")
+    ap.add_argument("--sweep-B", default="64,256,1024")
+    ap.add_argument("--sweep-G", default="1,8,16,32,64,128")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "haste" else args.warmup
 
+    if args.sweep:
+        run_sweep(args)
+        return
     from paper_2606_01117_b200 import synth
     cfg = synth.CONFIGS[args.workload]
     if args.impl == "reference":
