@@ -184,6 +184,11 @@ int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const vo
                cudaStream_t st, int* n_launches) {
   *n_launches = 1;
   static const bool use_red = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "red");   // first version, for comparison
+  static const bool use_mma = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "mma");
+  if (use_mma) {
+    const int rc = tc_tail_dx_mma(s, sh, idx, W, dY, dXt, st);
+    if (rc != HASTE_ERR_UNSUPPORTED) return rc;
+  }
 #define HASTE_DX(G_, K_)                                                                   \
   if (sh.G == G_ && sh.K == K_)                                                            \
     return use_red ? launch_dx_red<G_, K_>(s, sh, idx, W, dY, dXt, st) : tc_tail_dx_acc(s, sh, idx, W, dY, dXt, st)
