@@ -185,6 +185,11 @@ int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const vo
   *n_launches = 1;
   static const bool use_red = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "red");   // first version, for comparison
   static const bool use_mma = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "mma");
+  static const bool use_hyb = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "hyb");
+  if (use_hyb) {
+    const int rc = tc_tail_dx_hyb(s, sh, idx, W, dY, dXt, st);
+    if (rc != HASTE_ERR_UNSUPPORTED) return rc;
+  }
   if (use_mma) {
     const int rc = tc_tail_dx_mma(s, sh, idx, W, dY, dXt, st);
     if (rc != HASTE_ERR_UNSUPPORTED) return rc;

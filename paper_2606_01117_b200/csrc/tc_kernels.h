@@ -25,6 +25,9 @@ int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const vo
 // on-chip accumulating version (tc_dx_acc.cu)
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    cudaStream_t st);
+// tc_dx_acc with its TMEM class done by scatter MMAs (tc_dx_hyb.cu)
+int tc_tail_dx_hyb(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
+                   cudaStream_t st);
 // tensor cores do the scatter-add too (tc_dx_mma.cu)
 int tc_tail_dx_mma(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    cudaStream_t st);

@@ -102,11 +102,12 @@ def test_dx_classes_exact_and_close(oracle, case):
             assert oracle.rel_l2(out["dX"][:, lo:hi], ref["dX"][:, lo:hi]) <= 1e-4, (lo, hi)
 
 
-@pytest.mark.parametrize("kernel", ["red", "mma"])
+@pytest.mark.parametrize("kernel", ["red", "mma", "hyb"])
 def test_dx_other_kernels_still_match(kernel):
     """The first-version kernel (L2 reductions only, HASTE_DX_KERNEL=red) is kept as a comparison point, the experimental
-    one (HASTE_DX_KERNEL=mma: the scatter as a tf32 MMA reading P from TMEM) as groundwork: same answer, exactly, on
-    integers (|P| < 2048 is exact in tf32), unsorted and duplicated index rows included."""
+    ones (HASTE_DX_KERNEL=mma: the scatter as a tf32 MMA reading P from TMEM; =hyb: tc_dx_acc with only its TMEM class
+    done that way) as groundwork: same answer, exactly, on integers (|P| < 2048 is exact in tf32), unsorted and
+    duplicated index rows included, several groups per CTA (the plan rings wrap)."""
     import subprocess, sys, os, textwrap
     code = textwrap.dedent("""
         import numpy as np, sys
@@ -114,7 +115,7 @@ def test_dx_other_kernels_still_match(kernel):
         from paper_2606_01117_b200 import synth
         import oracle
         from gpu_util import TailRun
-        B, d, L, G, K = 200, 768, 64 * 9 + 3, 64, 128
+        B, d, L, G, K = 200, 768, 64 * 700 + 3, 64, 128
         inp = synth.small_case(77, B, d, L, G, K, dtype="bf16", with_bias=False, w_std=0.05)
         rng = np.random.RandomState(5)
         inp.idx[3] = np.sort(rng.choice(d, size=K, replace=True))      # duplicates
