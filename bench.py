@@ -452,8 +452,17 @@ def main():
         kernels["head_forward"]["TFLOP/s"] = head_f / (kernels["head_forward"]["ms"] * 1e-3) / 1e12
         kernels["head_backward"]["TFLOP/s"] = 2 * head_f / (kernels["head_backward"]["ms"] * 1e-3) / 1e12
     dom = max(("forward", "dW", "dX"), key=lambda k: kernels[k]["ms"])
+    # DRAM bytes per launch of that kernel from the committed ncu --set full capture (profiles/ncu_traffic.json); null for other workloads
+    traffic = None
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        if tj.get("workload") == args.workload:
+            traffic = tj.get(dom)
+    except Exception:
+        traffic = None
     roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["GB/s"], "peak": peaks["hbm"], "unit": "GB/s",
-                "frac": kernels[dom]["GB/s"] / peaks["hbm"], "traffic": None, "peak_source": peaks["source"] + " (burst copy)",
+                "frac": kernels[dom]["GB/s"] / peaks["hbm"], "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)",
+                "algorithmic_bytes": ab[dom], "peak_source": peaks["source"] + " (burst copy)",
                 "share_of_step": kernels[dom]["ms"] / ms_step}
     h2d = hX.numel() * 2 + hrow.numel() * 4 + hcol.numel() * 4 + (hXh.numel() * 2 if use_head else 0)
     d2h = 8 + B * d * 4 * (2 if use_head else 1)
