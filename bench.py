@@ -215,6 +215,22 @@ def run_reference(args, cfg):
     }))
 
 
+def max_over_ranks(ms, dist, device):
+    """Device time of the slowest rank (the job is as fast as its slowest replica).  `dist` is torch.distributed (any
+    backend: nccl on the GPU box, gloo in the CPU tests) or None for a single process."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([float(ms)], device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_tflops(world, step_flops, ms_per_step):
+    """`value`: N independent replicas ("replicas only") each do step_flops per step; weak scaling."""
+    return world * step_flops / (ms_per_step * 1e-3) / 1e12
+
+
 def run_sweep(args):
     """--sweep: BASELINE.json config 5 (kernel sweep at fixed nnz): B in {64,256,1024}, d=768, L=670091, K=64,
     G in {1,8,16,32,64,128} (G=1 = ungrouped per-label fixed fan-in, the comparison kernel), uniform sorted idx, no head,
@@ -393,12 +409,7 @@ def main():
             fn()
         e1.record()
         barrier()
-        ms = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), dist, dev)
 
     for _ in range(args.warmup):
         step()
@@ -436,8 +447,8 @@ def main():
     tail_f, head_f = _flops(cfg)
     step_flops = 3 * tail_f + (3 * head_f if use_head else 0)
     ms_step = ms_total / args.steps
-    value = world * step_flops / (ms_step * 1e-3) / 1e12
-    e2e_value = world * step_flops / (ms_e2e / args.steps * 1e-3) / 1e12
+    value = whole_job_tflops(world, step_flops, ms_step)
+    e2e_value = whole_job_tflops(world, step_flops, ms_e2e / args.steps)
     ab = _alg_bytes(cfg)
     kernels = {}
     for k in ("forward", "dW", "dX"):
