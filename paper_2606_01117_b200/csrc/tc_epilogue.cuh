@@ -16,43 +16,72 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// Packed fp32 pairs (sm_100: one instruction, two lanes of fp32 math).  The epilogue is issue-bound, so the ops that
+// exist in packed form (mul, fma, add) are done two logits at a time; tanh, |.| and max stay scalar.
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+
 // 32 logits of one batch row: z -> dY (bf16x2 packed) and the row's loss terms.
 //   sigma(z) = 1/2 + 1/2 tanh(z/2)  (one MUFU op);  softplus(z) = max(z,0) - ln( sigma(|z|) ), and the
 //   logs of a tile are taken once on the PRODUCT of the factors sigma(|z|) in [1/2,1)  (<= 16 per chain).
 // SLOW: some label of this chunk is a positive of this row, or the chunk holds padding labels (>= L).
+// Chains: logit jj feeds R[jj & 3] and P[jj & 3] (pair (j, j+1) = the two lanes of packed chain (j >> 1) & 1).
 template <bool SLOW, bool BIAS>
 __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
                                       float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
-  float bv[4] = {0.f, 0.f, 0.f, 0.f};
+  uint64_t R2[2] = {pk2(R[0], R[1]), pk2(R[2], R[3])}, P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};
+  const uint64_t half2 = pk2(0.5f, 0.5f), hs2 = pk2(hs, hs);
+  uint64_t bv2[2] = {0ull, 0ull};
 #pragma unroll
   for (int j = 0; j < 32; j += 2) {
-    float dy[2];
     if (BIAS && (j & 3) == 0) {
       const float4 t4 = lds128f(sbias + j * 4);
-      bv[0] = t4.x; bv[1] = t4.y; bv[2] = t4.z; bv[3] = t4.w;
+      bv2[0] = pk2(t4.x, t4.y); bv2[1] = pk2(t4.z, t4.w);
     }
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      const int jj = j + u;
-      float z = __uint_as_float(v[jj]);
-      if (BIAS) z += bv[jj & 3];
-      const float t = tanh_approx(0.5f * z);
-      float d = fmaf(t, hs, hs);
-      float f = fmaf(fabsf(t), 0.5f, 0.5f);
-      float r = fmaxf(z, 0.f);
-      if (SLOW) {
-        const bool valid = jj < nvalid;
-        const bool y = (ymask >> jj) & 1u;
-        if (y) { d -= s; r -= z; }
-        if (!valid) { d = 0.f; f = 1.f; r = 0.f; }
-        if (zout && valid) zout[jj] = z;
-      }
-      dy[u] = d;
-      P[jj & 3] *= f;
-      R[jj & 3] += r;
+    uint64_t z2 = pk2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]));
+    if (BIAS) z2 = add2(z2, bv2[(j >> 1) & 1]);
+    float z0, z1, zh0, zh1;
+    upk2(z2, z0, z1);
+    upk2(mul2(z2, half2), zh0, zh1);
+    const float t0 = tanh_approx(zh0), t1 = tanh_approx(zh1);
+    float d0, d1;
+    upk2(fma2(pk2(t0, t1), hs2, hs2), d0, d1);
+    float f0 = fmaf(fabsf(t0), 0.5f, 0.5f), f1 = fmaf(fabsf(t1), 0.5f, 0.5f);
+    float r0 = fmaxf(z0, 0.f), r1 = fmaxf(z1, 0.f);
+    if (SLOW) {
+      const bool valid0 = j < nvalid, valid1 = j + 1 < nvalid;
+      if ((ymask >> j) & 1u) { d0 -= s; r0 -= z0; }
+      if ((ymask >> (j + 1)) & 1u) { d1 -= s; r1 -= z1; }
+      if (!valid0) { d0 = 0.f; f0 = 1.f; r0 = 0.f; }
+      if (!valid1) { d1 = 0.f; f1 = 1.f; r1 = 0.f; }
+      if (zout && valid0) zout[j] = z0;
+      if (zout && valid1) zout[j + 1] = z1;
     }
-    out[j >> 1] = pack_bf16x2(dy[0], dy[1]);
+    P2[(j >> 1) & 1] = mul2(P2[(j >> 1) & 1], pk2(f0, f1));
+    R2[(j >> 1) & 1] = add2(R2[(j >> 1) & 1], pk2(r0, r1));
+    out[j >> 1] = pack_bf16x2(d0, d1);
   }
+  upk2(R2[0], R[0], R[1]); upk2(R2[1], R[2], R[3]);
+  upk2(P2[0], P[0], P[1]); upk2(P2[1], P[2], P[3]);
 }
 
 }  // namespace tc
