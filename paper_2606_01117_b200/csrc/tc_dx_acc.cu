@@ -130,7 +130,13 @@ template <int N> __device__ __forceinline__ void dxa_chunk_t(uint32_t tp, uint32
   for (int u = 0; u < N; ++u) a[u] = dxa_tld1(tlane + dst[u]);
   tmem_ld_wait();
 #pragma unroll
-  for (int u = 0; u < N; ++u) dxa_tst1(tlane + dst[u], __float_as_uint(__uint_as_float(a[u]) + __uint_as_float(pv[u])));
+  for (int u = 0; u < N; u += 2) {            // packed add: two slots per instruction (the kernel is issue-bound)
+    uint64_t s2;
+    asm("{\n\t.reg .b64 x, y;\n\tmov.b64 x, {%1, %2};\n\tmov.b64 y, {%3, %4};\n\tadd.rn.f32x2 %0, x, y;\n\t}"
+        : "=l"(s2) : "r"(a[u]), "r"(a[u + 1]), "r"(pv[u]), "r"(pv[u + 1]));
+    dxa_tst1(tlane + dst[u], (uint32_t)s2);
+    dxa_tst1(tlane + dst[u + 1], (uint32_t)(s2 >> 32));
+  }
 }
 // one chunk of N slots of a shared-memory class: acc row (byte offset dst[u]), this thread's word += P column u
 template <int N> __device__ __forceinline__ void dxa_chunk_s(uint32_t tp, uint32_t lst, uint32_t sown) {
@@ -143,7 +149,13 @@ template <int N> __device__ __forceinline__ void dxa_chunk_s(uint32_t tp, uint32
   for (int u = 0; u < N; ++u) a[u] = dxa_lds32f(sown + dst[u]);
   tmem_ld_wait();
 #pragma unroll
-  for (int u = 0; u < N; ++u) dxa_sts32f(sown + dst[u], a[u] + __uint_as_float(pv[u]));
+  for (int u = 0; u < N; u += 2) {            // packed add: two slots per instruction
+    uint64_t s2;
+    asm("{\n\t.reg .b64 x, y;\n\tmov.b64 x, {%1, %2};\n\tmov.b64 y, {%3, %4};\n\tadd.rn.f32x2 %0, x, y;\n\t}"
+        : "=l"(s2) : "f"(a[u]), "f"(a[u + 1]), "r"(pv[u]), "r"(pv[u + 1]));
+    dxa_sts32f(sown + dst[u], __uint_as_float((uint32_t)s2));
+    dxa_sts32f(sown + dst[u + 1], __uint_as_float((uint32_t)(s2 >> 32)));
+  }
 }
 
 // 20 warps poll barriers here; a polling loop costs issue slots the working warps need, so back off between polls
