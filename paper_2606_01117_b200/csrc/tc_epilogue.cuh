@@ -40,19 +40,13 @@ __device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
   return r;
 }
 
-// 32 logits of one batch row: z -> dY (bf16x2 packed) and the row's loss terms.
-//   sigma(z) = 1/2 + 1/2 tanh(z/2)  (one MUFU op);  softplus(z) = max(z,0) - ln( sigma(|z|) ), and the
-//   logs of a tile are taken once on the PRODUCT of the factors sigma(|z|) in [1/2,1)  (<= 16 per chain).
-// SLOW: some label of this chunk is a positive of this row, or the chunk holds padding labels (>= L).
-// Chains: logit jj feeds R[jj & 3] and P[jj & 3] (pair (j, j+1) = the two lanes of packed chain (j >> 1) & 1).
-template <bool SLOW, bool BIAS>
-__device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
-                                      float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
-  uint64_t R2[2] = {pk2(R[0], R[1]), pk2(R[2], R[3])}, P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};
-  const uint64_t half2 = pk2(0.5f, 0.5f), hs2 = pk2(hs, hs);
+// 8 logits (J0 .. J0+7) of one batch row.  SL: one of them may be a positive of the row or a padding label (>= L).
+template <bool SL, bool BIAS, int J0>
+__device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s, uint64_t half2,
+                                     uint64_t hs2, uint64_t (&R2)[2], uint64_t (&P2)[2], uint32_t (&out)[16], float* zout) {
   uint64_t bv2[2] = {0ull, 0ull};
 #pragma unroll
-  for (int j = 0; j < 32; j += 2) {
+  for (int j = J0; j < J0 + 8; j += 2) {
     if (BIAS && (j & 3) == 0) {
       const float4 t4 = lds128f(sbias + j * 4);
       bv2[0] = pk2(t4.x, t4.y); bv2[1] = pk2(t4.z, t4.w);
@@ -67,7 +61,7 @@ __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, u
     upk2(fma2(pk2(t0, t1), hs2, hs2), d0, d1);
     float f0 = fmaf(fabsf(t0), 0.5f, 0.5f), f1 = fmaf(fabsf(t1), 0.5f, 0.5f);
     float r0 = fmaxf(z0, 0.f), r1 = fmaxf(z1, 0.f);
-    if (SLOW) {
+    if (SL) {
       const bool valid0 = j < nvalid, valid1 = j + 1 < nvalid;
       if ((ymask >> j) & 1u) { d0 -= s; r0 -= z0; }
       if ((ymask >> (j + 1)) & 1u) { d1 -= s; r1 -= z1; }
@@ -80,6 +74,30 @@ __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, u
     R2[(j >> 1) & 1] = add2(R2[(j >> 1) & 1], pk2(r0, r1));
     out[j >> 1] = pack_bf16x2(d0, d1);
   }
+}
+
+// 32 logits of one batch row: z -> dY (bf16x2 packed) and the row's loss terms.
+//   sigma(z) = 1/2 + 1/2 tanh(z/2)  (one MUFU op);  softplus(z) = max(z,0) - ln( sigma(|z|) ), and the
+//   logs of a tile are taken once on the PRODUCT of the factors sigma(|z|) in [1/2,1)  (<= 16 per chain).
+// SLOW: some label of this chunk may be a positive of some row of the warp, or the chunk holds padding labels (>= L), or
+// logits are wanted; the decision is then refined per 8 logits (warp-uniform), because the special-case code costs more
+// than the math itself and positives are rare (in the dense head ~70 % of the (warp, 128-label tile) pairs hold one).
+// Chains: logit jj feeds R[jj & 3] and P[jj & 3] (pair (j, j+1) = the two lanes of packed chain (j >> 1) & 1).
+template <bool SLOW, bool BIAS>
+__device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
+                                      float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
+  uint64_t R2[2] = {pk2(R[0], R[1]), pk2(R[2], R[3])}, P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};
+  const uint64_t half2 = pk2(0.5f, 0.5f), hs2 = pk2(hs, hs);
+#define HASTE_EPI8(J0_)                                                                                             \
+  if (SLOW) {                                                                                                        \
+    const bool sl = __any_sync(0xffffffffu, ((ymask >> J0_) & 0xffu) != 0u) || nvalid < J0_ + 8 || zout != nullptr; \
+    if (sl) epi8<true, BIAS, J0_>(v, sbias, ymask, nvalid, s, half2, hs2, R2, P2, out, zout);                        \
+    else epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                              \
+  } else {                                                                                                           \
+    epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                                   \
+  }
+  HASTE_EPI8(0) HASTE_EPI8(8) HASTE_EPI8(16) HASTE_EPI8(24)
+#undef HASTE_EPI8
   upk2(R2[0], R[0], R[1]); upk2(R2[1], R[2], R[3]);
   upk2(P2[0], P[0], P[1]); upk2(P2[1], P[2], P[3]);
 }

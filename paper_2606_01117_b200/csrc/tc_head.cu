@@ -9,6 +9,7 @@
 // Every operand is read in the layout it has in HBM: a transposed operand is an MN-major UMMA descriptor, not a copy.
 // warp roles (192 threads): warps 0-3 epilogue (thread = accumulator row), warp 4 MMA issuer, warp 5 TMA loader.
 #include <algorithm>
+#include <cstdint>
 #include <cstring>
 #include <new>
 
@@ -189,6 +190,8 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const uint32_t sbias_w = sbase + C::OFF_BIAS + q * 512;
     float loss_local = 0.f;
     int n = 0, nstore = 0;
+    int cur_row = -1, cur_n0 = 0, pc = 0, pe = 0;             // CSR cursor of the forward epilogue
+    int64_t nxt = INT64_MAX;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       const HeadItem wi = head_item(p, w);
       if (wi.kb1 <= wi.kb0) continue;
@@ -199,15 +202,26 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 
       if (MODE == HEAD_FWD) {
         const bool valid_row = row < p.B;
+        // positives of this row inside the tile.  A CTA's tiles keep their m tile (grid % MT == 0) and move up in n, so the
+        // thread keeps a cursor into its CSR row (sorted columns) instead of re-scanning the row for every tile (that
+        // scan, one dependent load per positive, was 15 of the kernel's 42 us); any other tile order resets the cursor.
         uint32_t ym[4] = {0u, 0u, 0u, 0u};
         if (valid_row && p.rowptr) {
-          const int r0 = __ldg(p.rowptr + row), r1 = __ldg(p.rowptr + row + 1);
-          for (int pp = r0; pp < r1; ++pp) {
-            const int64_t o = (int64_t)__ldg(p.col + pp) - p.label_offset - n0;
-            if (o >= 0 && o < BN && n0 + o < p.L) {
+          if (row != cur_row || n0 < cur_n0) {
+            cur_row = row;
+            pc = __ldg(p.rowptr + row); pe = __ldg(p.rowptr + row + 1);
+            nxt = pc < pe ? (int64_t)__ldg(p.col + pc) - p.label_offset : INT64_MAX;
+          }
+          cur_n0 = n0;
+          const int64_t hi = min((int64_t)n0 + BN, p.L);
+          while (nxt < hi) {
+            const int64_t o = nxt - n0;
+            if (o >= 0) {
 #pragma unroll
               for (int i = 0; i < 4; ++i) if ((int)(o >> 5) == i) ym[i] |= 1u << (o & 31);
             }
+            ++pc;
+            nxt = pc < pe ? (int64_t)__ldg(p.col + pc) - p.label_offset : INT64_MAX;
           }
         }
         const int nl = (int)min((int64_t)BN, p.L - n0);
@@ -225,17 +239,18 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const float hs = 0.5f * p.s;
         float R[4] = {0.f, 0.f, 0.f, 0.f}, P[4] = {1.f, 1.f, 1.f, 1.f};
         float lt = 0.f;
-#pragma unroll
+#pragma unroll 1                 // one copy of the epilogue code: unrolled four times it overflows the instruction cache
         for (int sc = 0; sc < 4; ++sc) {
           uint32_t v[32];
+          const uint32_t ymsc = sc == 0 ? ym[0] : sc == 1 ? ym[1] : sc == 2 ? ym[2] : ym[3];
           tmem_ld32(taddr + sc * 32, v);
           tmem_ld_wait();
           uint32_t out[16];
           float* zout = (p.logits && valid_row) ? p.logits + (size_t)row * p.L + n0 + sc * 32 : nullptr;
           const uint32_t sb = sbias_w + sc * 128;
           if (slow) {
-            if (p.bias) epi32<true, true>(v, sb, ym[sc], nl - sc * 32, p.s, hs, R, P, out, zout);
-            else epi32<true, false>(v, sb, ym[sc], nl - sc * 32, p.s, hs, R, P, out, zout);
+            if (p.bias) epi32<true, true>(v, sb, ymsc, nl - sc * 32, p.s, hs, R, P, out, zout);
+            else epi32<true, false>(v, sb, ymsc, nl - sc * 32, p.s, hs, R, P, out, zout);
           } else {
             if (p.bias) epi32<false, true>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
             else epi32<false, false>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
