@@ -453,8 +453,8 @@ int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, cons
     if constexpr (DxAccCfg<G_, K_, 3>::FITS) if (nst == 3) return launch_dx_acc<G_, K_, 3>(s, sh, idx, W, dY, dXt, st);  \
     return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, st);                                       \
   }
-  HASTE_DXA(64, 128, 3); HASTE_DXA(64, 64, 3); HASTE_DXA(128, 64, 3); HASTE_DXA(128, 128, 2);
-  HASTE_DXA(32, 64, 3); HASTE_DXA(32, 128, 3);
+  HASTE_DXA(64, 128, 2); HASTE_DXA(64, 64, 2); HASTE_DXA(128, 64, 2); HASTE_DXA(128, 128, 2);
+  HASTE_DXA(32, 64, 2); HASTE_DXA(32, 128, 2);
 #undef HASTE_DXA
   return HASTE_ERR_UNSUPPORTED;
 }
