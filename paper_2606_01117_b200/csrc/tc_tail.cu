@@ -289,8 +289,12 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * G;
       float R[4] = {0.f, 0.f, 0.f, 0.f}, P[4] = {1.f, 1.f, 1.f, 1.f};
       uint32_t v[32];                 // one chunk at a time: 16 epilogue warps hide the TMEM latency, registers are short
-#pragma unroll
+      // two chunks are unrolled; four copies of the epilogue code (G = 128) overflow the instruction cache (see tc_head.cu)
+#pragma unroll(G >= 128 ? 1 : 2)
       for (int sc = 0; sc < G / 32; ++sc) {
+        uint32_t ymsc = ym[0];
+#pragma unroll
+        for (int i = 1; i < G / 32; ++i) if (sc == i) ymsc = ym[i];
         tmem_ld32(taddr + sc * 32, v);
         tmem_ld_wait();
         if (sc + 1 == G / 32) {
@@ -304,8 +308,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         const int nvalid = nl - sc * 32;
         const uint32_t sb = sbias_w + sc * 128;
         if (slow) {
-          if (p.bias) epi32<true, true>(v, sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
-          else epi32<true, false>(v, sb, ym[sc], nvalid, p.s, hs, R, P, out, zout);
+          if (p.bias) epi32<true, true>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
+          else epi32<true, false>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
         } else {
           if (p.bias) epi32<false, true>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
           else epi32<false, false>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
