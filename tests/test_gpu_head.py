@@ -79,6 +79,36 @@ def test_head_parity(oracle, case, force_simt):
     assert oracle.rel_l2(dX2.cpu().numpy() - 1.0, bref["dX"]) <= max(tol, 1e-4)
 
 
+@pytest.mark.parametrize("B,Lh", [(512, 128 * 100), (300, 128 * 120 + 40)])
+def test_head_many_tiles_per_cta_heavy_rows(oracle, B, Lh):
+    """Several output tiles per CTA and 40 positives per row: the forward epilogue keeps a cursor into each CSR row while
+    a CTA's tiles move up in n with a fixed m tile (B = 512: 4 m tiles, 148 % 4 == 0) and resets it when the m tile
+    changes from tile to tile (B = 300: 3 m tiles).  dY at the positive pairs is the gate that sees the targets."""
+    from paper_2606_01117_b200 import haste
+    d = 256
+    X, W, bias, rowptr, col, bits = _case(7 + B, B, d, Lh, "bf16", True, n_pos=40, L_total=Lh + 500)
+    dev = torch.device("cuda:0")
+    head = haste.HasteHead(d, Lh, B, "bf16")
+    assert head.kernel_family == 1
+    loss = torch.full((1,), float("nan"), device=dev)
+    dY = torch.full((B, Lh), float("nan"), dtype=head.tdtype, device=dev)
+    head.forward_loss(B, _dev(X, bits["X"]), _dev(W, bits["W"]), _dev(bias), _dev(rowptr), _dev(col), loss=loss, dY=dY)
+    ref = oracle.head_forward(X, W, bias, rowptr, col)
+    assert abs(loss.item() - ref["loss"]) <= 5e-3 * abs(ref["loss"])
+    dYn = dY.float().cpu().numpy()
+    assert oracle.rel_l2(dYn, ref["dY"]) <= 5e-3
+    rows = np.repeat(np.arange(B), np.diff(rowptr))
+    keep = col < Lh
+    assert keep.sum() > 30 * B
+    assert oracle.rel_l2(dYn[rows[keep], col[keep]], ref["dY"][rows[keep], col[keep]]) <= 5e-3
+    # every positive moved dY by -s: a missed or misplaced target shows as an error of the order of s = 1/B
+    s = 1.0 / B
+    assert np.max(np.abs(dYn[rows[keep], col[keep]] - ref["dY"][rows[keep], col[keep]])) < 0.02 * s
+    neg = np.ones((B, Lh), dtype=bool)
+    neg[rows[keep], col[keep]] = False
+    assert np.max(np.abs(dYn[neg] - ref["dY"][neg])) < 0.02 * s
+
+
 def test_head_empty():
     from paper_2606_01117_b200 import haste
     dev = torch.device("cuda:0")
