@@ -311,6 +311,7 @@ def main():
     ap.add_argument("--workload", default=WORKLOAD, help="synth.CONFIGS key (default: the 670K-label config the metric is quoted on)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-head", action="store_true", help="time the sparse tail alone")
+    ap.add_argument("--deterministic", action="store_true", help="create the handles with HASTE_DETERMINISTIC (atomic-free dX)")
     ap.add_argument("--sweep", action="store_true", help="config 5: kernel sweep over B and G at K=64 against the dense bottleneck (one JSON line per point)")
     ap.add_argument("--sweep-B", default="64,256,1024")
     ap.add_argument("--sweep-G", default="1,8,16,32,64,128")
@@ -351,7 +352,8 @@ def main():
     hX, hrow, hcol = bf(inp.bits["X"]).pin_memory(), torch.from_numpy(inp.rowptr).pin_memory(), torch.from_numpy(inp.col).pin_memory()
     X, rowptr, col = hX.to(dev), hrow.to(dev), hcol.to(dev)
     W, idx = bf(inp.bits["W"]).to(dev), torch.from_numpy(inp.idx).to(dev)
-    layer = haste.HasteLayer(d, L, G, K, B, "bf16", label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT, device=local)
+    det = haste.HASTE_DETERMINISTIC if args.deterministic else 0
+    layer = haste.HasteLayer(d, L, G, K, B, "bf16", label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT | det, device=local)
     layer.validate_index(idx)
     dY = layer.alloc_dy(B)
     dW = torch.empty(L, K, dtype=torch.bfloat16, device=dev)
@@ -361,7 +363,7 @@ def main():
     if use_head:
         hXh = bf(inp.bits["X_head"]).pin_memory()
         Xh, Wh = hXh.to(dev), bf(inp.bits["W_head"]).to(dev)
-        head = haste.HasteHead(d, Lh, B, "bf16", label_offset=0, device=local)
+        head = haste.HasteHead(d, Lh, B, "bf16", label_offset=0, flags=det, device=local)
         dYh = torch.empty(B, Lh, dtype=torch.bfloat16, device=dev)
         dWh = torch.empty(Lh, d, dtype=torch.bfloat16, device=dev)
         dbh = torch.empty(Lh, device=dev)
@@ -483,7 +485,7 @@ def main():
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "config3_670k" if args.workload == "670k" else args.workload, "B": B, "d": d, "L_tail": L, "L_head": Lh if use_head else 0,
                    "G": G, "K": K, "replicas": world, "l2": "inputs larger than L2 (per pass W %d MB + dY %d MB vs 126 MB L2); no explicit flush" % (L * K * 2 >> 20, cfg.NG * G * B * 2 >> 20),
-                   "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}},
+                   "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}, "deterministic": bool(args.deterministic)},
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": int(n_launch), "clocks": clocks, "roofline": roofline, "kernels": kernels,
         "loss": [float(v) for v in loss.cpu().tolist()],

@@ -66,7 +66,9 @@ typedef enum { HASTE_F32 = 0, HASTE_BF16 = 1 } haste_dtype_t;
 
 typedef enum {
   HASTE_IDX_SORTED_DISTINCT = 1u, /* promise: every idx row strictly ascending */
-  HASTE_DETERMINISTIC = 2u,       /* forbid float atomics on dX (slower path) */
+  HASTE_DETERMINISTIC = 2u,       /* no float atomics on dX: bit-identical results from run to run (slower path; the sparse tail
+                                     needs a shape of the tcgen05 family for it, else haste_create returns HASTE_ERR_UNSUPPORTED;
+                                     costs a workspace of num_SMs * d * 512 bytes) */
   HASTE_FORCE_SIMT = 4u           /* use the generic CUDA-core kernels even where tcgen05 kernels exist */
 } haste_flags_t;
 

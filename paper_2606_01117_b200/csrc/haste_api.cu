@@ -87,6 +87,7 @@ struct haste_layer {
   int Bpad;         // row pitch of Xt / dXt
   void* Xt;         // [d][Bpad] dtype
   float* dXt;       // [d][Bpad] fp32
+  float* dx_part;   // HASTE_DETERMINISTIC: [num_sms][d][128] fp32 private partial tiles of the dX kernel, else null
   double* loss_acc; // device scalar
   float* partials;  // [n_partials] per-CTA loss partials (tcgen05 family)
   int n_partials;
@@ -142,10 +143,6 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
     set_error("haste_create: unknown dtype");
     return HASTE_ERR_INVALID_ARG;
   }
-  if (cfg->flags & HASTE_DETERMINISTIC) {
-    set_error("haste_create: HASTE_DETERMINISTIC (atomic-free dX) is not implemented yet");
-    return HASTE_ERR_UNSUPPORTED;
-  }
   if (cfg->G > 1024 || cfg->K > 4096) {
     set_error("haste_create: G <= 1024 and K <= 4096 are supported");
     return HASTE_ERR_UNSUPPORTED;
@@ -190,6 +187,20 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
     if (rc != HASTE_OK) { haste_destroy(h); return rc; }
     h->family = 1;
   }
+  if (cfg->flags & HASTE_DETERMINISTIC) {
+    // atomic-free dX: only the accumulating tcgen05 kernel has such a variant (private partial tiles + ordered reduction)
+    if (h->family != 1) {
+      set_error("haste_create: HASTE_DETERMINISTIC needs a shape of the tcgen05 family (bf16, G in {32,64,128}, K in {64,128})");
+      haste_destroy(h);
+      return HASTE_ERR_UNSUPPORTED;
+    }
+    const size_t part_bytes = (size_t)tc_tail_num_sms(h->tc) * cfg->d * 128 * 4;
+    if (cudaMalloc(&h->dx_part, part_bytes) != cudaSuccess) {
+      set_error("haste_create: allocation of the deterministic dX workspace (%zu bytes) failed", part_bytes);
+      haste_destroy(h);
+      return HASTE_ERR_NOMEM;
+    }
+  }
   *out = h;
   return HASTE_OK;
 }
@@ -199,7 +210,7 @@ int haste_destroy(haste_layer_t* h) {
   DeviceGuard guard(h->device);
   if (h->tc) tc_tail_destroy(h->tc);
   if (h->prof) { h->prof->destroy(); delete h->prof; }
-  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag);
+  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->dx_part); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag);
   delete h;
   return HASTE_OK;
 }
@@ -350,7 +361,16 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
     rc = HASTE_ERR_UNSUPPORTED;
     if (h->family == 1) {
       int n = 0;
-      rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, st, &n);
+      if (h->dx_part) {
+        int NT = 0, S = 0;
+        tc_tail_dx_grid(h->tc, sh, &NT, &S);
+        HASTE_CUDA_TRY(cudaMemsetAsync(h->dx_part, 0, (size_t)NT * S * sh.d * 128 * 4, st));
+        rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, h->dx_part, st, &n);
+        if (rc == HASTE_OK) { rc = launch_reduce_dx_parts(h->dx_part, h->dXt, sh.d, h->Bpad, NT, S, st); ++n; }
+        if (rc == HASTE_ERR_UNSUPPORTED) { set_error("haste_backward: no atomic-free dX kernel for this call"); return rc; }
+      } else {
+        rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, nullptr, st, &n);
+      }
       if (rc == HASTE_OK) h->last_launches += n;
     }
     if (rc == HASTE_ERR_UNSUPPORTED) {
@@ -535,7 +555,7 @@ int haste_head_backward(haste_head_t* h, int B, const void* X, const void* Wh, c
   pf.begin(HASTE_KERNEL_DW, st);     // the head's backward is timed as one unit (dW, db and dX)
   if (h->family == 1) {
     int n = 0;
-    int rc = tc_head_backward(h->tc, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, st, &n);
+    int rc = tc_head_backward(h->tc, sh, X, Wh, dY, dWh, dbias, dX, accumulate_dX, (h->flags & HASTE_DETERMINISTIC) ? 1 : 0, st, &n);
     if (rc) return rc;
     h->last_launches += n;
   } else {

@@ -180,9 +180,19 @@ static int launch_dx_red(TcTailState* s, const TailShape& sh, const int32_t* idx
   return HASTE_OK;
 }
 
+void tc_tail_dx_grid(const TcTailState* s, const TailShape& sh, int* NT, int* S) {
+  *NT = ceil_div(sh.B, 128);
+  *S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / *NT));
+}
+int tc_tail_num_sms(const TcTailState* s) { return s->num_sms; }
+
 int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-               cudaStream_t st, int* n_launches) {
+               float* dx_part, cudaStream_t st, int* n_launches) {
   *n_launches = 1;
+  if (dx_part) {   // deterministic mode: only the accumulating kernel has an atomic-free variant
+    if ((sh.G == 32 || sh.G == 64 || sh.G == 128) && (sh.K == 64 || sh.K == 128)) return tc_tail_dx_acc(s, sh, idx, W, dY, dXt, dx_part, st);
+    return HASTE_ERR_UNSUPPORTED;
+  }
   static const bool use_red = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "red");   // first version, for comparison
   static const bool use_mma = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "mma");
   static const bool use_hyb = getenv("HASTE_DX_KERNEL") && !strcmp(getenv("HASTE_DX_KERNEL"), "hyb");
@@ -196,10 +206,10 @@ int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const vo
   }
 #define HASTE_DX(G_, K_)                                                                   \
   if (sh.G == G_ && sh.K == K_)                                                            \
-    return use_red ? launch_dx_red<G_, K_>(s, sh, idx, W, dY, dXt, st) : tc_tail_dx_acc(s, sh, idx, W, dY, dXt, st)
+    return use_red ? launch_dx_red<G_, K_>(s, sh, idx, W, dY, dXt, st) : tc_tail_dx_acc(s, sh, idx, W, dY, dXt, nullptr, st)
   HASTE_DX(64, 128); HASTE_DX(64, 64); HASTE_DX(128, 64); HASTE_DX(128, 128);
 #undef HASTE_DX
-  if (sh.G == 32 && (sh.K == 64 || sh.K == 128)) return tc_tail_dx_acc(s, sh, idx, W, dY, dXt, st);   // 64-byte-swizzle operand: acc kernel only
+  if (sh.G == 32 && (sh.K == 64 || sh.K == 128)) return tc_tail_dx_acc(s, sh, idx, W, dY, dXt, nullptr, st);   // 64-byte-swizzle operand: acc kernel only
   return HASTE_ERR_UNSUPPORTED;
 }
 

@@ -40,6 +40,8 @@ struct DxAccParams {
   int B, Bpad, NT, S, d;
   int64_t NG;
   int fa, f1, fb, f2;   // class boundaries (see above)
+  float* part;          // HASTE_DETERMINISTIC: private partial tiles [grid][d][128] fp32 (zeroed by the caller) instead of
+                        // reductions into dXt; null otherwise.  See the note at the L class below.
 };
 
 template <int G, int K, int NST_> struct DxAccCfg {
@@ -163,7 +165,7 @@ template <int NS_SLEEP> __device__ __forceinline__ void dxa_wait(uint64_t* bar, 
   while (!mbar_try_wait(bar, parity)) __nanosleep(NS_SLEEP);
 }
 
-template <int G, int K, int NST>
+template <int G, int K, int NST, bool DET>
 __global__ void __launch_bounds__(DxAccCfg<G, K, NST>::THREADS, 1)
 tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmW, const DxAccParams p) {
   using C = DxAccCfg<G, K, NST>;
@@ -242,6 +244,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     // j - lo of that class's list, so every lane writes its own PER entries; no gather, no second pass.
     constexpr int PER = K / 32;
     const int aw = warp - (4 * C::NSET + 2);
+    const int lrow_bytes = DET ? 512 : p.Bpad * 4;
     int e[PER], en[PER];
 #pragma unroll
     for (int t = 0; t < PER; ++t) { e[t] = 0; en[t] = 0; }
@@ -284,6 +287,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         sts32(ring + 16, (uint32_t)c2);
         sts32(ring + 20, (uint32_t)ca); sts32(ring + 24, (uint32_t)(cb - c1)); sts32(ring + 28, (uint32_t)(c1 - ca));
         sts32(ring + 32, (uint32_t)(c2 - cb)); sts32(ring + 36, (uint32_t)(K - c2));
+        sts32(ring + 40, strict ? 1u : 0u);
       }
 #pragma unroll
       for (int t = 0; t < PER; ++t) {
@@ -293,7 +297,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         else if (j < c1) { l = 2; k = j - ca; code = 2 * K + f; }
         else if (j < cb) { l = 1; k = j - c1; code = (f - p.f1) * 512; }          // byte offset of the accumulator row
         else if (j < c2) { l = 3; k = j - cb; code = (f - p.f1) * 512; }
-        else             { l = 4; k = j - c2; code = f * p.Bpad * 4; }            // byte offset of the dX^T row
+        else             { l = 4; k = j - c2; code = f * lrow_bytes; }           // byte offset of the dX^T (or private tile) row
         sts32(lists + (l * C::LIST_LEN + k) * 4, (uint32_t)code);
       }
       // pad the on-chip lists to a whole chunk with the class's dummy destination
@@ -315,8 +319,11 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     const bool vb = b < p.B;
     const uint32_t tlane = tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t sown = sbase + C::OFF_ACC + row * 4;                      // + accumulator row * 512
-    float* const gcol = p.dXt + b;                                           // + f * Bpad
-    const char* const gbytes = reinterpret_cast<const char*>(gcol);          // + byte offset of the dX^T row (L list code)
+    // atomic mode: column b of dX^T (row pitch Bpad); deterministic mode: column `row` of this CTA's private tile (pitch 128)
+    constexpr bool det = DET;                                                // a template parameter: the default kernel pays nothing for it
+    const size_t gpitch = det ? 128 : (size_t)p.Bpad;
+    float* const gcol = det ? p.part + (size_t)blockIdx.x * p.d * 128 + row : p.dXt + b;   // + f * gpitch
+    char* const gbytes = reinterpret_cast<char*>(gcol);                      // + byte offset of the row (L list code)
     // this set's own accumulators: [c_lo, c_hi) TMEM columns (relative to the lane base) or shared-memory rows
     const int c_lo = set == 0 ? 2 * K : set == 2 ? 2 * K + p.fa : set == 1 ? 0 : p.fb - p.f1;
     const int c_hi = set == 0 ? 2 * K + p.fa : set == 2 ? 2 * K + p.f1 : set == 1 ? p.fb - p.f1 : NS;
@@ -360,13 +367,30 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
       // target here: a shared dummy word in L2 would serialise the reductions of every CTA on one address.
       const uint32_t lstl = lists + C::NSET * C::LIST_LEN * 4;
 #pragma unroll 1
-      for (int m = l_first * 16; m < n_l; m += C::NSET * 16) {
+      // Deterministic mode: plain read-modify-write of the private tile.  A word (f, b) must then have ONE writer at a time:
+      // set 3 alone takes every L chunk, and the flush below waits for it behind a barrier.  The order of additions into a
+      // word is then fixed: groups in order, then the owner's flush, then the stripes in order (reduce kernel).
+      for (int m = det ? (set == 3 ? 0 : n_l) : l_first * 16; m < n_l; m += det ? 16 : C::NSET * 16) {
         uint32_t pv[16];
         int dst[16];
         tmem_ld16(tp + lo_l + m, pv);
         dxa_load_dest<16>(lstl + m * 4, dst);
         tmem_ld_wait();
-        if (vb) {
+        if (vb && det) {
+          if (dxa_lds32i(ring + 40)) {        // strictly increasing row: 16 distinct words, loads first, then stores
+            float a[16];
+#pragma unroll
+            for (int u = 0; u < 16; ++u)
+              if (m + u < n_l) asm volatile("ld.global.f32 %0, [%1];" : "=f"(a[u]) : "l"(gbytes + (uint32_t)dst[u]) : "memory");
+#pragma unroll
+            for (int u = 0; u < 16; ++u)
+              if (m + u < n_l) asm volatile("st.global.f32 [%0], %1;" ::"l"(gbytes + (uint32_t)dst[u]), "f"(a[u] + __uint_as_float(pv[u])) : "memory");
+          } else {                            // duplicates possible: one word at a time
+#pragma unroll
+            for (int u = 0; u < 16; ++u)
+              if (m + u < n_l) { volatile float* a = reinterpret_cast<volatile float*>(gbytes + (uint32_t)dst[u]); *a = *a + __uint_as_float(pv[u]); }
+          }
+        } else if (vb) {
           if (m + 16 <= n_l) {
 #pragma unroll
             for (int u = 0; u < 16; ++u) dxa_red_add_f32(gbytes + (uint32_t)dst[u], __uint_as_float(pv[u]));
@@ -382,6 +406,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
       if (lane == 0) { mbar_arrive(&t_empty[slot]); mbar_arrive(&d_empty[r]); }
     }
     // flush this thread's accumulators (its batch row of every feature this set owns) into dX^T
+    if (det) named_bar_sync(1, 4 * C::NSET * 32);       // set 3 has finished its read-modify-writes of the private tile
     if (is_t) {
       dxa_tmem_st_wait();
       for (int c0 = c_lo; c0 < c_hi; c0 += 16) {
@@ -392,11 +417,17 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         if (vb) {
 #pragma unroll
           for (int u = 0; u < 16; ++u)
-            if (c0 + u < c_hi) dxa_red_add_f32(gcol + (size_t)(c0 + u - 2 * K) * p.Bpad, __uint_as_float(v[u]));
+            if (c0 + u < c_hi) {
+              float* a = gcol + (size_t)(c0 + u - 2 * K) * gpitch;
+              if (det) *a += __uint_as_float(v[u]); else dxa_red_add_f32(a, __uint_as_float(v[u]));
+            }
         }
       }
     } else if (vb) {
-      for (int r = c_lo; r < c_hi; ++r) dxa_red_add_f32(gcol + (size_t)(p.f1 + r) * p.Bpad, dxa_lds32f(sown + r * 512));
+      for (int r = c_lo; r < c_hi; ++r) {
+        float* a = gcol + (size_t)(p.f1 + r) * gpitch;
+        if (det) *a += dxa_lds32f(sown + r * 512); else dxa_red_add_f32(a, dxa_lds32f(sown + r * 512));
+      }
     }
   }
 
@@ -407,7 +438,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
 
 template <int G, int K, int NST>
 static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-                         cudaStream_t st) {
+                         float* part, cudaStream_t st) {
   using C = DxAccCfg<G, K, NST>;
   CUtensorMap tmY, tmW;
   {
@@ -425,7 +456,7 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
     if (rc) return rc;
   }
   DxAccParams p;
-  p.dXt = dXt; p.idx = idx; p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NG = sh.NG; p.d = sh.d;
+  p.dXt = dXt; p.part = part; p.idx = idx; p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NG = sh.NG; p.d = sh.d;
   if (p.NT > s->num_sms) return HASTE_ERR_UNSUPPORTED;
   if ((int64_t)sh.d * sh.Bpad * 4 > 0x7fffffff) return HASTE_ERR_UNSUPPORTED;   // list codes are 32-bit byte offsets
   p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NT));
@@ -436,22 +467,27 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   ns = std::min(ns, sh.d - f1);
   p.f1 = f1; p.fa = f1 / 2; p.f2 = f1 + ns; p.fb = f1 + ns / 2;
   const int smem = C::OFF_ACC + (ns + 1) * 512 + 1024;
-  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K, NST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  tc_dx_acc_kernel<G, K, NST><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+  if (part) {
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K, NST, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    tc_dx_acc_kernel<G, K, NST, true><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+  } else {
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K, NST, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    tc_dx_acc_kernel<G, K, NST, false><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+  }
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }
 
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-                   cudaStream_t st) {
+                   float* part, cudaStream_t st) {
   // operand stages: as many as leave room for a useful number of shared-memory accumulator rows
   static const int nst_env = getenv("HASTE_DX_NST") ? atoi(getenv("HASTE_DX_NST")) : 0;
 #define HASTE_DXA(G_, K_, DEF_)                                                                       \
   if (sh.G == G_ && sh.K == K_) {                                                                     \
     const int nst = nst_env ? nst_env : DEF_;                                                         \
-    if constexpr (DxAccCfg<G_, K_, 4>::FITS) if (nst == 4) return launch_dx_acc<G_, K_, 4>(s, sh, idx, W, dY, dXt, st);  \
-    if constexpr (DxAccCfg<G_, K_, 3>::FITS) if (nst == 3) return launch_dx_acc<G_, K_, 3>(s, sh, idx, W, dY, dXt, st);  \
-    return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, st);                                       \
+    if constexpr (DxAccCfg<G_, K_, 4>::FITS) if (nst == 4) return launch_dx_acc<G_, K_, 4>(s, sh, idx, W, dY, dXt, part, st);  \
+    if constexpr (DxAccCfg<G_, K_, 3>::FITS) if (nst == 3) return launch_dx_acc<G_, K_, 3>(s, sh, idx, W, dY, dXt, part, st);  \
+    return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, part, st);                                       \
   }
   HASTE_DXA(64, 128, 2); HASTE_DXA(64, 64, 2); HASTE_DXA(128, 64, 2); HASTE_DXA(128, 128, 2);
   HASTE_DXA(32, 64, 2); HASTE_DXA(32, 128, 2);

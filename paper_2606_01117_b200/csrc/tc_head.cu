@@ -421,7 +421,7 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
 }
 
 int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const void* dY, void* dWh,
-                     float* dbias, float* dX, int accumulate_dX, cudaStream_t st, int* n_launches) {
+                     float* dbias, float* dX, int accumulate_dX, int deterministic, cudaStream_t st, int* n_launches) {
   *n_launches = 0;
   if (dWh || dbias) {
     CUtensorMap tmA, tmB, tmO;
@@ -445,7 +445,8 @@ int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const v
     if (rc) return rc;
     HeadParams p = base_params(sh);
     p.MT = ceil_div(sh.B, 128); p.NTL = ceil_div(sh.d, HeadCfg<HEAD_DX>::BN); p.KB = ceil_div(sh.L, 64);
-    p.NSLAB = std::max(1, std::min(p.KB, s->num_sms / (p.MT * p.NTL)));
+    // split over label slabs, partial tiles added with cp.reduce (float atomics): one slab when determinism is asked for
+    p.NSLAB = deterministic ? 1 : std::max(1, std::min(p.KB, s->num_sms / (p.MT * p.NTL)));
     rc = launch_head<HEAD_DX>(s, tmA, tmB, tmO, p, st);
     if (rc) return rc;
     ++*n_launches;

@@ -20,11 +20,16 @@ int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const i
                     float* logits_out, cudaStream_t st, int* n_launches);
 int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
                float* dbias, cudaStream_t st, int* n_launches);
+// dx_part: null, or (HASTE_DETERMINISTIC) private partial tiles [tc_tail_dx_parts()][d][128] fp32, zeroed by the caller: the kernel
+// then uses no float atomics and the caller sums the tiles of a batch tile in stripe order (launch_reduce_dx_parts)
 int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-               cudaStream_t st, int* n_launches);
+               float* dx_part, cudaStream_t st, int* n_launches);
+// grid of the dX kernel for this batch size: NT batch tiles x S stripes (CTA = stripe * NT + batch tile)
+void tc_tail_dx_grid(const TcTailState* s, const TailShape& sh, int* NT, int* S);
+int tc_tail_num_sms(const TcTailState* s);
 // on-chip accumulating version (tc_dx_acc.cu)
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-                   cudaStream_t st);
+                   float* part, cudaStream_t st);
 // tc_dx_acc with its TMEM class done by scatter MMAs (tc_dx_hyb.cu)
 int tc_tail_dx_hyb(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    cudaStream_t st);
@@ -40,6 +45,6 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
                     const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
                     cudaStream_t st, int* n_launches);
 int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const void* dY, void* dWh,
-                     float* dbias, float* dX, int accumulate_dX, cudaStream_t st, int* n_launches);
+                     float* dbias, float* dX, int accumulate_dX, int deterministic, cudaStream_t st, int* n_launches);
 
 }  // namespace haste

@@ -70,6 +70,19 @@ int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, 
   return HASTE_OK;
 }
 
+// HASTE_DETERMINISTIC: dXt[f][bt*128 + r] = sum over stripes s (in order) of part[s*NT + bt][f][r]   (tc_dx_acc.cu private tiles)
+__global__ void reduce_dx_parts_kernel(const float* __restrict__ part, float* __restrict__ dXt, int d, int Bpad, int NT, int S) {
+  const int r = threadIdx.x, f = blockIdx.x, bt = blockIdx.y;
+  float v = 0.f;
+  for (int s = 0; s < S; ++s) v += part[((size_t)(s * NT + bt) * d + f) * 128 + r];
+  dXt[(size_t)f * Bpad + bt * 128 + r] = v;
+}
+int launch_reduce_dx_parts(const float* part, float* dXt, int d, int Bpad, int NT, int S, cudaStream_t st) {
+  reduce_dx_parts_kernel<<<dim3(d, NT), 128, 0, st>>>(part, dXt, d, Bpad, NT, S);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
 // loss = scale * (acc + sum(partials[0..n)))  -- one thread, fixed order: deterministic.
 __global__ void finalize_loss_kernel(const double* acc, const float* partials, int n, float scale, float* loss) {
   __shared__ double red[256];
