@@ -437,6 +437,8 @@ def main():
     layer.set_profiling(0)
     if use_head:
         head.set_profiling(0)
+    # the same K steps once more with the library's per-kernel events off: what the instrumentation of the timed region costs
+    ms_plain = timed(step, args.steps)
     for _ in range(2):
         step_e2e()
     ms_e2e = timed(step_e2e, args.steps)
@@ -488,6 +490,8 @@ def main():
                    "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}, "deterministic": bool(args.deterministic)},
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": int(n_launch), "clocks": clocks, "roofline": roofline, "kernels": kernels,
+        "events_off": {"ms_per_step": ms_plain / args.steps, "value": whole_job_tflops(world, step_flops, ms_plain / args.steps),
+                       "note": "same K steps repeated without the per-kernel CUDA events that the timed region carries"},
         "loss": [float(v) for v in loss.cpu().tolist()],
     }
     if not args.no_cpu_baseline and world == 1:
