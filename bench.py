@@ -368,47 +368,79 @@ def main():
         dWh = torch.empty(Lh, d, dtype=torch.bfloat16, device=dev)
         dbh = torch.empty(Lh, device=dev)
         dXh = torch.empty(B, d, device=dev)
-    h_loss = torch.zeros(2).pin_memory()
-    h_dX = torch.empty(B, d).pin_memory()
-    h_dXh = torch.empty(B, d).pin_memory()
     launches = [0]
 
-    def step():
+    class Batch:
+        """Device buffers of one step's inputs and results.  The device-resident runs use batch 0; the end-to-end run
+        alternates between two, so that the copies of one step overlap the kernels of its neighbours."""
+        def __init__(self, first):
+            self.X, self.rowptr, self.col = (X, rowptr, col) if first else (torch.empty_like(X), torch.empty_like(rowptr), torch.empty_like(col))
+            self.dX, self.loss = (dX, loss) if first else (torch.empty_like(dX), torch.zeros_like(loss))
+            if use_head:
+                self.Xh, self.dXh = (Xh, dXh) if first else (torch.empty_like(Xh), torch.empty_like(dXh))
+            self.h_loss, self.h_dX, self.h_dXh = torch.zeros(2).pin_memory(), torch.empty(B, d).pin_memory(), torch.empty(B, d).pin_memory()
+            self.ev_in, self.ev_done, self.ev_out = torch.cuda.Event(), torch.cuda.Event(), torch.cuda.Event()
+
+    batches = [Batch(True), Batch(False)]
+    s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+
+    def step(b=batches[0]):
         n = 0
-        layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY)
+        layer.forward_loss(B, b.X, idx, W, None, b.rowptr, b.col, loss=b.loss[0:1], dY=dY)
         n += layer.last_launch_count
-        layer.backward(B, X, idx, W, dY, dW=dW, dbias=db, dX=dX)
+        layer.backward(B, b.X, idx, W, dY, dW=dW, dbias=db, dX=b.dX)
         n += layer.last_launch_count
         if use_head:
-            head.forward_loss(B, Xh, Wh, None, rowptr, col, loss=loss[1:2], dY=dYh)
+            head.forward_loss(B, b.Xh, Wh, None, b.rowptr, b.col, loss=b.loss[1:2], dY=dYh)
             n += head.last_launch_count
-            head.backward(B, Xh, Wh, dYh, dWh=dWh, dbias=dbh, dX=dXh)
+            head.backward(B, b.Xh, Wh, dYh, dWh=dWh, dbias=dbh, dX=b.dXh)
             n += head.last_launch_count
         launches[0] += n
 
+    e2e_count = [0]
+
     def step_e2e():
-        X.copy_(hX, non_blocking=True)
-        rowptr.copy_(hrow, non_blocking=True)
-        col.copy_(hcol, non_blocking=True)
-        if use_head:
-            Xh.copy_(hXh, non_blocking=True)
-        step()
-        h_loss.copy_(loss, non_blocking=True)
-        h_dX.copy_(dX, non_blocking=True)
-        if use_head:
-            h_dXh.copy_(dXh, non_blocking=True)
+        # one step end to end: inputs from pinned host memory, results back to pinned host memory, through the public
+        # calls.  Three streams (copy in, kernels, copy out) and two batches: every step still does all of its copies.
+        b = batches[e2e_count[0] & 1]
+        e2e_count[0] += 1
+        main = torch.cuda.current_stream()
+        with torch.cuda.stream(s_in):
+            s_in.wait_event(b.ev_done)          # the kernels of the step that last used this batch have read its inputs
+            b.X.copy_(hX, non_blocking=True)
+            b.rowptr.copy_(hrow, non_blocking=True)
+            b.col.copy_(hcol, non_blocking=True)
+            if use_head:
+                b.Xh.copy_(hXh, non_blocking=True)
+            b.ev_in.record(s_in)
+        main.wait_event(b.ev_in)
+        main.wait_event(b.ev_out)               # the results of that earlier step have left the batch
+        step(b)
+        b.ev_done.record(main)
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(b.ev_done)
+            b.h_loss.copy_(b.loss, non_blocking=True)
+            b.h_dX.copy_(b.dX, non_blocking=True)
+            if use_head:
+                b.h_dXh.copy_(b.dXh, non_blocking=True)
+            b.ev_out.record(s_out)
+
+    def finish_e2e():
+        torch.cuda.current_stream().wait_stream(s_out)   # the closing event of the timed region comes after the last copy out
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(fn, steps):
+    def timed(fn, steps, finish=None):
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         for _ in range(steps):
             fn()
+        if finish is not None:
+            finish()
         e1.record()
         barrier()
         return max_over_ranks(e0.elapsed_time(e1), dist, dev)
@@ -441,7 +473,11 @@ def main():
     ms_plain = timed(step, args.steps)
     for _ in range(2):
         step_e2e()
-    ms_e2e = timed(step_e2e, args.steps)
+    ms_e2e = timed(step_e2e, args.steps, finish_e2e)
+    # the pipelined run must have brought back the results of the device-resident run (same inputs every step)
+    for b in batches:
+        if not torch.equal(b.h_loss, loss.cpu()) or not torch.allclose(b.h_dX, dX.cpu(), rtol=1e-3, atol=1e-6):
+            raise RuntimeError("bench.py: the end-to-end run returned different results from the device-resident run")
 
     if rank != 0:
         if dist is not None:
