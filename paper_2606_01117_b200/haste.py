@@ -118,6 +118,7 @@ class HasteLayer:
                                   label_offset=label_offset, loss_scale=loss_scale, flags=flags)
         self.device = device
         self.h = ctypes.c_void_p()
+        self._destroy = lib().haste_destroy      # bound here: module globals may be gone when __del__ runs at interpreter exit
         _check(lib().haste_create(ctypes.byref(self.h), ctypes.byref(self.cfg), device))
         self.NG = -(-L // G)
         self.tdtype = _TORCH[self.cfg.dtype]
@@ -125,8 +126,8 @@ class HasteLayer:
 
     def close(self):
         if getattr(self, "h", None) is not None and self.h.value:
-            lib().haste_destroy(self.h)
-            self.h = ctypes.c_void_p()
+            self._destroy(self.h)
+            self.h = None
 
     __del__ = close
 
@@ -179,13 +180,14 @@ class HasteHead:
         self.dtype = _dt(dtype)
         self.tdtype = _TORCH[self.dtype]
         self.h = ctypes.c_void_p()
+        self._destroy = lib().haste_head_destroy
         _check(lib().haste_head_create(ctypes.byref(self.h), d, L_h, B_max, self.dtype, label_offset, loss_scale, flags,
                                        device))
 
     def close(self):
         if getattr(self, "h", None) is not None and self.h.value:
-            lib().haste_head_destroy(self.h)
-            self.h = ctypes.c_void_p()
+            self._destroy(self.h)
+            self.h = None
 
     __del__ = close
 
