@@ -33,12 +33,14 @@ def _flops(cfg):
     return tail, head
 
 
-def _alg_bytes(cfg, dw_bytes=2):
+def _alg_bytes(cfg, dw_bytes=None):
     """Algorithmic HBM bytes per launch of each tail kernel."""
-    W = cfg.L_t * cfg.K * 2
+    e = 2 if cfg.dtype == "bf16" else 4          # element size of X, W, dY (and dW unless stated)
+    dw_bytes = e if dw_bytes is None else dw_bytes
+    W = cfg.L_t * cfg.K * e
     idx = cfg.NG * cfg.K * 4
-    dY = cfg.NG * cfg.G * cfg.B * 2
-    X = cfg.B * cfg.d * 2
+    dY = cfg.NG * cfg.G * cfg.B * e
+    X = cfg.B * cfg.d * e
     dX = cfg.B * cfg.d * 4
     return {
         "forward": W + idx + X + dY,
@@ -346,26 +348,31 @@ def main():
     B, d, L, G, K, Lh = cfg.B, cfg.d, cfg.L_t, cfg.G, cfg.K, cfg.L_h
     use_head = (not args.no_head) and Lh > 0
 
-    def bf(bits):
-        return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+    tdt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
+    esz = 2 if cfg.dtype == "bf16" else 4
 
-    hX, hrow, hcol = bf(inp.bits["X"]).pin_memory(), torch.from_numpy(inp.rowptr).pin_memory(), torch.from_numpy(inp.col).pin_memory()
+    def host(key):    # the values both sides consume: bf16 bit patterns (bf16 configs) or the fp32 array (config 1)
+        if key in inp.bits:
+            return torch.from_numpy(np.ascontiguousarray(inp.bits[key]).view(np.int16)).view(torch.bfloat16)
+        return torch.from_numpy(np.ascontiguousarray(getattr(inp, key), dtype=np.float32))
+
+    hX, hrow, hcol = host("X").pin_memory(), torch.from_numpy(inp.rowptr).pin_memory(), torch.from_numpy(inp.col).pin_memory()
     X, rowptr, col = hX.to(dev), hrow.to(dev), hcol.to(dev)
-    W, idx = bf(inp.bits["W"]).to(dev), torch.from_numpy(inp.idx).to(dev)
+    W, idx = host("W").to(dev), torch.from_numpy(inp.idx).to(dev)
     det = haste.HASTE_DETERMINISTIC if args.deterministic else 0
-    layer = haste.HasteLayer(d, L, G, K, B, "bf16", label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT | det, device=local)
+    layer = haste.HasteLayer(d, L, G, K, B, cfg.dtype, label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT | det, device=local)
     layer.validate_index(idx)
     dY = layer.alloc_dy(B)
-    dW = torch.empty(L, K, dtype=torch.bfloat16, device=dev)
+    dW = torch.empty(L, K, dtype=tdt, device=dev)
     db = torch.empty(L, device=dev)
     dX = torch.empty(B, d, device=dev)
     loss = torch.zeros(2, device=dev)
     if use_head:
-        hXh = bf(inp.bits["X_head"]).pin_memory()
-        Xh, Wh = hXh.to(dev), bf(inp.bits["W_head"]).to(dev)
-        head = haste.HasteHead(d, Lh, B, "bf16", label_offset=0, flags=det, device=local)
-        dYh = torch.empty(B, Lh, dtype=torch.bfloat16, device=dev)
-        dWh = torch.empty(Lh, d, dtype=torch.bfloat16, device=dev)
+        hXh = host("X_head").pin_memory()
+        Xh, Wh = hXh.to(dev), host("W_head").to(dev)
+        head = haste.HasteHead(d, Lh, B, cfg.dtype, label_offset=0, flags=det, device=local)
+        dYh = torch.empty(B, Lh, dtype=tdt, device=dev)
+        dWh = torch.empty(Lh, d, dtype=tdt, device=dev)
         dbh = torch.empty(Lh, device=dev)
         dXh = torch.empty(B, d, device=dev)
     launches = [0]
@@ -515,16 +522,22 @@ def main():
                 "frac": kernels[dom]["GB/s"] / peaks["hbm"], "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)",
                 "algorithmic_bytes": ab[dom], "peak_source": peaks["source"] + " (burst copy)",
                 "share_of_step": kernels[dom]["ms"] / ms_step}
-    h2d = hX.numel() * 2 + hrow.numel() * 4 + hcol.numel() * 4 + (hXh.numel() * 2 if use_head else 0)
+    pass_mb = (L * K * esz >> 20, cfg.NG * G * B * esz >> 20)
+    if sum(pass_mb) > 126:
+        l2_note = "inputs larger than L2 (per pass W %d MB + dY %d MB vs 126 MB L2); no explicit flush" % pass_mb
+    else:
+        l2_note = "inputs SMALLER than L2 (per pass W %d MB + dY %d MB vs 126 MB L2) and no flush: an L2-resident parity-size config, not a roofline measurement" % pass_mb
+    h2d = hX.numel() * esz + hrow.numel() * 4 + hcol.numel() * 4 + (hXh.numel() * esz if use_head else 0)
     d2h = 8 + B * d * 4 * (2 if use_head else 1)
     out = {
         "metric": "sparse_layer_fwd_bwd_tflops_670k", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
+        "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": "config3_670k" if args.workload == "670k" else args.workload, "B": B, "d": d, "L_tail": L, "L_head": Lh if use_head else 0,
-                   "G": G, "K": K, "replicas": world, "l2": "inputs larger than L2 (per pass W %d MB + dY %d MB vs 126 MB L2); no explicit flush" % (L * K * 2 >> 20, cfg.NG * G * B * 2 >> 20),
+                   "G": G, "K": K, "replicas": world, "l2": l2_note,
                    "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}, "deterministic": bool(args.deterministic)},
-        "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "note": "copies on their own streams, two sets of device buffers; no per-kernel events in this run (compare with events_off)"},
         "gpu_launches": int(n_launch), "clocks": clocks, "roofline": roofline, "kernels": kernels,
         "events_off": {"ms_per_step": ms_plain / args.steps, "value": whole_job_tflops(world, step_flops, ms_plain / args.steps),
                        "note": "same K steps repeated without the per-kernel CUDA events that the timed region carries"},
