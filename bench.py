@@ -510,10 +510,10 @@ def main():
         kernels["head_forward"]["TFLOP/s"] = head_f / (kernels["head_forward"]["ms"] * 1e-3) / 1e12
         kernels["head_backward"]["TFLOP/s"] = 2 * head_f / (kernels["head_backward"]["ms"] * 1e-3) / 1e12
     dom = max(("forward", "dW", "dX"), key=lambda k: kernels[k]["ms"])
-    # DRAM bytes per launch of that kernel from the committed ncu --set full capture (profiles/ncu_traffic.json); null for other workloads
+    # DRAM bytes per launch of that kernel from the committed ncu --set full capture (profiles/r01_ncu_traffic.txt); null for other workloads
     traffic = None
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_ncu_traffic.txt")))
         if tj.get("workload") == args.workload:
             traffic = tj.get(dom)
     except Exception:
