@@ -194,6 +194,12 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
       haste_destroy(h);
       return HASTE_ERR_UNSUPPORTED;
     }
+    // one private tile per CTA of the dX kernel: its grid is NT * S <= num_SMs, which needs NT = ceil(B/128) <= num_SMs
+    if ((cfg->B_max + 127) / 128 > tc_tail_num_sms(h->tc)) {
+      set_error("haste_create: HASTE_DETERMINISTIC supports B_max <= %d", 128 * tc_tail_num_sms(h->tc));
+      haste_destroy(h);
+      return HASTE_ERR_UNSUPPORTED;
+    }
     const size_t part_bytes = (size_t)tc_tail_num_sms(h->tc) * cfg->d * 128 * 4;
     if (cudaMalloc(&h->dx_part, part_bytes) != cudaSuccess) {
       set_error("haste_create: allocation of the deterministic dX workspace (%zu bytes) failed", part_bytes);
@@ -364,6 +370,7 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
       if (h->dx_part) {
         int NT = 0, S = 0;
         tc_tail_dx_grid(h->tc, sh, &NT, &S);
+        if (NT * S > tc_tail_num_sms(h->tc)) { set_error("haste_backward: batch too large for the deterministic dX workspace"); return HASTE_ERR_UNSUPPORTED; }
         HASTE_CUDA_TRY(cudaMemsetAsync(h->dx_part, 0, (size_t)NT * S * sh.d * 128 * 4, st));
         rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, h->dx_part, st, &n);
         if (rc == HASTE_OK) { rc = launch_reduce_dx_parts(h->dx_part, h->dXt, sh.d, h->Bpad, NT, S, st); ++n; }

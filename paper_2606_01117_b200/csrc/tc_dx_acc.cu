@@ -15,7 +15,7 @@
 //     L  = [f2, d)                   red.global.add.f32 into dX^T, as in the first version (tc_dx.cu)
 // A CTA owns (128-row batch tile, stripe of groups).  Per group: TMA loads the dY tile and W_g, one thread
 // issues P^T[128 batch x K slots] = dY tile * W_g (tcgen05, fp32 in TMEM, double buffered), an auxiliary
-// warp (one of four, round-robin) turns idx_g into one destination list per class, and 16 epilogue warps (4 sets x 4 TMEM lane
+// warp (one of two, alternating groups) turns idx_g into one destination list per class, and 16 epilogue warps (4 sets x 4 TMEM lane
 // quadrants; a lane owns one batch row) add column j of P into the destination of slot j.  Set s owns class s
 // exclusively, so no two threads ever touch the same accumulator word and nothing on chip is atomic; the L
 // chunks (atomic in L2, hence owner-free) are dealt round-robin to the four sets, shared-memory sets first
@@ -26,7 +26,6 @@
 // legal by DESIGN.md reading R4) take the L path for every slot, which is correct for any index row.
 // The accumulators are flushed into dX^T once per CTA.
 #include <algorithm>
-#include <cstdlib>
 
 #include "tc_common.cuh"
 #include "tc_kernels.h"
@@ -460,11 +459,9 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   if (p.NT > s->num_sms) return HASTE_ERR_UNSUPPORTED;
   if ((int64_t)sh.d * sh.Bpad * 4 > 0x7fffffff) return HASTE_ERR_UNSUPPORTED;   // list codes are 32-bit byte offsets
   p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NT));
-  // class sizes: what fits (tuning knobs for experiments: HASTE_DX_F1, HASTE_DX_NS)
-  int f1 = std::min(sh.d, C::TF), ns = C::NS_MAX;
-  if (const char* e = getenv("HASTE_DX_F1")) f1 = std::max(0, std::min(f1, atoi(e)));
-  if (const char* e = getenv("HASTE_DX_NS")) ns = std::max(0, std::min(ns, atoi(e)));
-  ns = std::min(ns, sh.d - f1);
+  // class sizes: what fits
+  const int f1 = std::min(sh.d, C::TF);
+  const int ns = std::min(C::NS_MAX, sh.d - f1);
   p.f1 = f1; p.fa = f1 / 2; p.f2 = f1 + ns; p.fb = f1 + ns / 2;
   const int smem = C::OFF_ACC + (ns + 1) * 512 + 1024;
   if (part) {
@@ -480,17 +477,11 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
 
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    float* part, cudaStream_t st) {
-  // operand stages: as many as leave room for a useful number of shared-memory accumulator rows
-  static const int nst_env = getenv("HASTE_DX_NST") ? atoi(getenv("HASTE_DX_NST")) : 0;
-#define HASTE_DXA(G_, K_, DEF_)                                                                       \
-  if (sh.G == G_ && sh.K == K_) {                                                                     \
-    const int nst = nst_env ? nst_env : DEF_;                                                         \
-    if constexpr (DxAccCfg<G_, K_, 4>::FITS) if (nst == 4) return launch_dx_acc<G_, K_, 4>(s, sh, idx, W, dY, dXt, part, st);  \
-    if constexpr (DxAccCfg<G_, K_, 3>::FITS) if (nst == 3) return launch_dx_acc<G_, K_, 3>(s, sh, idx, W, dY, dXt, part, st);  \
-    return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, part, st);                                       \
-  }
-  HASTE_DXA(64, 128, 2); HASTE_DXA(64, 64, 2); HASTE_DXA(128, 64, 2); HASTE_DXA(128, 128, 2);
-  HASTE_DXA(32, 64, 2); HASTE_DXA(32, 128, 2);
+  // two operand stages: more were measured to gain nothing and they cost shared-memory accumulator rows
+#define HASTE_DXA(G_, K_) \
+  if (sh.G == G_ && sh.K == K_) return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, part, st)
+  HASTE_DXA(64, 128); HASTE_DXA(64, 64); HASTE_DXA(128, 64); HASTE_DXA(128, 128);
+  HASTE_DXA(32, 64); HASTE_DXA(32, 128);
 #undef HASTE_DXA
   return HASTE_ERR_UNSUPPORTED;
 }

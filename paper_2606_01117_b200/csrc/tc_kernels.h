@@ -30,12 +30,6 @@ int tc_tail_num_sms(const TcTailState* s);
 // on-chip accumulating version (tc_dx_acc.cu)
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    float* part, cudaStream_t st);
-// tc_dx_acc with its TMEM class done by scatter MMAs (tc_dx_hyb.cu)
-int tc_tail_dx_hyb(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-                   cudaStream_t st);
-// tensor cores do the scatter-add too (tc_dx_mma.cu)
-int tc_tail_dx_mma(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
-                   cudaStream_t st);
 
 bool tc_head_supported(int d, int64_t L_h, int B_max, haste_dtype_t dtype, int device);
 int tc_head_create(TcHeadState** out, int d, int64_t L_h, int B_max, int device);
