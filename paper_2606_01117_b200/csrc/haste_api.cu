@@ -168,7 +168,7 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
   h->Bpad = round_up(cfg->B_max, 128);
   h->n_partials = 1024;
   const size_t xt_bytes = (size_t)cfg->d * h->Bpad * esize(cfg->dtype);
-  const size_t dxt_bytes = (size_t)cfg->d * round_up(cfg->B_max, 256) * 4;   // dX^T [d][Bpad], or the pair kernel's [B/256][d][128][2]
+  const size_t dxt_bytes = (size_t)cfg->d * h->Bpad * 4;
   cudaError_t e = cudaMalloc(&h->Xt, xt_bytes);
   if (e == cudaSuccess) e = cudaMalloc(&h->dXt, dxt_bytes);
   if (e == cudaSuccess) e = cudaMalloc(&h->loss_acc, sizeof(double));
@@ -345,8 +345,7 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
     if (rc) return rc;
     h->last_launches++;
   }
-  const bool dx_pair = dX && h->family == 1 && !h->dx_part && tc_tail_dx_pair_supported(sh);
-  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, dx_pair ? (size_t)sh.d * round_up(B, 256) * 4 : (size_t)sh.d * h->Bpad * 4, st));
+  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
   pf.end(HASTE_KERNEL_PREP_BWD, st);
   if (dW || dbias) {
     pf.begin(HASTE_KERNEL_DW, st);
@@ -366,18 +365,6 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
   if (dX) {
     pf.begin(HASTE_KERNEL_DX, st);
     rc = HASTE_ERR_UNSUPPORTED;
-    if (dx_pair) {
-      rc = tc_tail_dx_pair(h->tc, sh, idx, W, dY, h->dXt, st);
-      if (rc) return rc;
-      h->last_launches++;
-      pf.end(HASTE_KERNEL_DX, st);
-      pf.begin(HASTE_KERNEL_POST_BWD, st);
-      rc = launch_dxw_to_dx(h->dXt, dX, B, sh.d, accumulate_dX, st);
-      if (rc) return rc;
-      h->last_launches++;
-      pf.end(HASTE_KERNEL_POST_BWD, st);
-      return HASTE_OK;
-    }
     if (h->family == 1) {
       int n = 0;
       if (h->dx_part) {

@@ -10,8 +10,6 @@ namespace haste {
 int launch_transpose_pad(haste_dtype_t dt, const void* X, void* Xt, int B, int d, int Bpad, int Bzero, cudaStream_t st);
 // dX[b][f] (=|+=) dXt[f][b]
 int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st);
-// dX[b][f] (=|+=) dXw[b / 256][f][b % 128][(b % 256) / 128]   (workspace layout of tc_dx_pair.cu)
-int launch_dxw_to_dx(const float* dXw, float* dX, int B, int d, int accumulate, cudaStream_t st);
 int launch_reduce_dx_parts(const float* part, float* dXt, int d, int Bpad, int NT, int S, cudaStream_t st);
 int launch_finalize_loss(const double* acc, const float* partials, int n_partials, float scale, float* loss, cudaStream_t st);
 int launch_dy_unpack(haste_dtype_t dt, const void* dY, float* out_BL, int B, int64_t L, int G, cudaStream_t st);

@@ -209,7 +209,6 @@ struct TcTailState {
   haste_config_t cfg;
   int device, num_sms, Bpad;
   int n_partials;
-  int pair_clusters;   // tc_dx_pair.cu: co-resident clusters of its kernel (0 = not asked yet)
 };
 
 }  // namespace haste

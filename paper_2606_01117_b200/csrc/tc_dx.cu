@@ -2,12 +2,9 @@
 //
 //   dX[:, idx_g] += dY_g [B x G] * W_g [G x K]   over all groups g
 //
-// Two kernels implement it, both keeping the reduction over a CTA's groups on chip:
-//   tc_dx_pair.cu  two CTAs of a cluster share one stream of (256-row batch tile, group) units, each owning half of
-//                  the feature range; a thread owns TWO batch rows, so every accumulator instruction carries two adds
-//                  (the default when the batch has more than 128 rows)
-//   tc_dx_acc.cu   one CTA per (128-row batch tile, stripe of groups); also the HASTE_DETERMINISTIC variant
-// The choice depends on the shape only, never on the environment.
+// One kernel implements it (tc_dx_acc.cu: one CTA per (128-row batch tile, stripe of groups), the reduction over the
+// CTA's groups kept on chip; also the HASTE_DETERMINISTIC variant).  The choice depends on the shape only, never on
+// the environment.  DESIGN.md section 5 records the round-2 two-CTA-cluster kernel that was built, measured and dropped.
 #include <algorithm>
 
 #include "tc_common.cuh"

@@ -164,6 +164,16 @@ template <int NS_SLEEP> __device__ __forceinline__ void dxa_wait(uint64_t* bar, 
   while (!mbar_try_wait(bar, parity)) __nanosleep(NS_SLEEP);
 }
 
+// wait for two barriers at once: both phase checks are in flight together (a check costs 100-300 cycles even when it succeeds)
+__device__ __forceinline__ void dxa_wait2(uint64_t* a, uint32_t pa, uint64_t* b, uint32_t pb) {
+  bool da = false, db = false;
+  do {
+    const bool ta = da || mbar_try_wait(a, pa);
+    const bool tb = db || mbar_try_wait(b, pb);
+    da = ta; db = tb;
+  } while (!(da && db));
+}
+
 template <int G, int K, int NST, bool DET>
 __global__ void __launch_bounds__(DxAccCfg<G, K, NST>::THREADS, 1)
 tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmW, const DxAccParams p) {
@@ -222,8 +232,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::Y_BYTES, G * 128, 1024);
     for (int i = 0; i < n_my; ++i) {
       const int st = i % C::NST, slot = i & 1;
-      mbar_wait(&full[st], (i / C::NST) & 1);
-      mbar_wait(&t_empty[slot], ((i >> 1) & 1) ^ 1);
+      dxa_wait2(&full[st], (i / C::NST) & 1, &t_empty[slot], ((i >> 1) & 1) ^ 1);
       tc_fence_after();
       if (elect_one()) {
         const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
@@ -336,13 +345,12 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     }
     for (int i = 0; i < n_my; ++i) {
       const int r = i % C::RD, slot = i & 1;
-      dxa_wait<64>(&d_full[r], (i / C::RD) & 1);
+      dxa_wait2(&d_full[r], (i / C::RD) & 1, &t_full[slot], (i >> 1) & 1);
+      tc_fence_after();
       const uint32_t ring = sbase + C::OFF_RING + r * C::RING_BYTES;
       const uint32_t lists = ring + C::RING_META;
       const int lo_s = dxa_lds32i(ring + set * 4), n_s = dxa_lds32i(ring + 20 + set * 4);
       const int lo_l = dxa_lds32i(ring + C::NSET * 4), n_l = dxa_lds32i(ring + 20 + C::NSET * 4);
-      dxa_wait<64>(&t_full[slot], (i >> 1) & 1);
-      tc_fence_after();
       const uint32_t tp = tlane + slot * K;
       const uint32_t lst = lists + set * C::LIST_LEN * 4;
       if (is_t) {

@@ -31,12 +31,6 @@ int tc_tail_num_sms(const TcTailState* s);
 int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                    float* part, cudaStream_t st);
 
-// two-CTA-cluster version with two batch rows per thread (tc_dx_pair.cu); output in the workspace layout
-// dXw [ceil(B/256)][d][128][2] fp32 (zeroed by the caller), turned into dX by launch_dxw_to_dx
-bool tc_tail_dx_pair_supported(const TailShape& sh);
-int tc_tail_dx_pair(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXw,
-                    cudaStream_t st);
-
 bool tc_head_supported(int d, int64_t L_h, int B_max, haste_dtype_t dtype, int device);
 int tc_head_create(TcHeadState** out, int d, int64_t L_h, int B_max, int device);
 void tc_head_destroy(TcHeadState* s);

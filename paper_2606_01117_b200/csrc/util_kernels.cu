@@ -70,35 +70,6 @@ int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, 
   return HASTE_OK;
 }
 
-// dX[b][f] (=|+=) dXw[b / 256][f][b % 128][(b % 256) / 128]: the pair kernel's thread owns rows (r, r + 128) of a 256-row tile
-__global__ void dxw_to_dx_kernel(const float* __restrict__ dXw, float* __restrict__ dX, int B, int d, int accumulate) {
-  __shared__ float tile[32][33];
-  const int b0 = blockIdx.x * 32, f0 = blockIdx.y * 32;
-  const int tx = threadIdx.x, ty = threadIdx.y;
-#pragma unroll
-  for (int r = ty; r < 32; r += 8) {
-    const int f = f0 + r, b = b0 + tx;
-    tile[r][tx] = (f < d && b < B) ? dXw[(((int64_t)(b >> 8) * d + f) * 128 + (b & 127)) * 2 + ((b >> 7) & 1)] : 0.f;
-  }
-  __syncthreads();
-#pragma unroll
-  for (int r = ty; r < 32; r += 8) {
-    const int b = b0 + r, f = f0 + tx;
-    if (b < B && f < d) {
-      float v = tile[tx][r];
-      float* q = dX + (int64_t)b * d + f;
-      if (accumulate) v += *q;
-      *q = v;
-    }
-  }
-}
-int launch_dxw_to_dx(const float* dXw, float* dX, int B, int d, int accumulate, cudaStream_t st) {
-  dim3 grid(ceil_div(B, 32), ceil_div(d, 32)), block(32, 8);
-  dxw_to_dx_kernel<<<grid, block, 0, st>>>(dXw, dX, B, d, accumulate);
-  HASTE_LAUNCH_CHECK();
-  return HASTE_OK;
-}
-
 // HASTE_DETERMINISTIC: dXt[f][bt*128 + r] = sum over stripes s (in order) of part[s*NT + bt][f][r]   (tc_dx_acc.cu private tiles)
 __global__ void reduce_dx_parts_kernel(const float* __restrict__ part, float* __restrict__ dXt, int d, int Bpad, int NT, int S) {
   const int r = threadIdx.x, f = blockIdx.x, bt = blockIdx.y;

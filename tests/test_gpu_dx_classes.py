@@ -103,9 +103,9 @@ def test_dx_classes_exact_and_close(oracle, case):
 
 
 # ---------------------------------------------------------------------------------------------------------------
-# tc_dx_pair.cu (batches of more than 128 rows): two CTAs of a cluster split the feature range at ceil(d / 2); inside
-# a CTA's half the features are T (TMEM), S (shared memory), L (workspace reductions) by id; a CTA's slots are cut
-# into jobs of 48; a pair walks a contiguous range of (256-row tile, group) units and flushes when the tile changes.
+# Batches of several 128-row tiles with index rows that put whole groups into one half of the feature range, one slot
+# apart from the rest, runs across the middle of the range, duplicates and unsorted rows, and enough groups that a
+# CTA's stripe holds many of them (written for the round-2 cluster kernel, kept as parity cases of the product kernel).
 # ---------------------------------------------------------------------------------------------------------------
 def _pair_idx(rng, NG, K, d, kind):
     half = (d + 1) // 2
@@ -154,7 +154,7 @@ PAIR_CASES = [
 
 
 @pytest.mark.parametrize("case", PAIR_CASES, ids=lambda c: "B%d_d%d_NG%d_G%d_K%d_%s" % c)
-def test_dx_pair_exact_and_close(oracle, case):
+def test_dx_multi_tile_exact_and_close(oracle, case):
     from paper_2606_01117_b200 import haste
     from gpu_util import TailRun, dy_rounded
     B, d, NG, G, K, kind = case
