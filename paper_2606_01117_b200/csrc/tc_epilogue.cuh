@@ -40,7 +40,24 @@ __device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
   return r;
 }
 
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float r;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+  return r;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 // 8 logits (J0 .. J0+7) of one batch row.  SL: one of them may be a positive of the row or a padding label (>= L).
+// sigma(z) = 1/2 + 1/2 tanh.approx(z/2), one MUFU op per logit (the caller has checked that this is good enough, see epi32).
 template <bool SL, bool BIAS, int J0>
 __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s, uint64_t half2,
                                      uint64_t hs2, uint64_t (&R2)[2], uint64_t (&P2)[2], uint32_t (&out)[16], float* zout) {
@@ -53,13 +70,13 @@ __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, ui
     }
     uint64_t z2 = pk2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]));
     if (BIAS) z2 = add2(z2, bv2[(j >> 1) & 1]);
-    float z0, z1, zh0, zh1;
+    float z0, z1, d0, d1, f0, f1;
     upk2(z2, z0, z1);
+    float zh0, zh1;
     upk2(mul2(z2, half2), zh0, zh1);
     const float t0 = tanh_approx(zh0), t1 = tanh_approx(zh1);
-    float d0, d1;
     upk2(fma2(pk2(t0, t1), hs2, hs2), d0, d1);
-    float f0 = fmaf(fabsf(t0), 0.5f, 0.5f), f1 = fmaf(fabsf(t1), 0.5f, 0.5f);
+    f0 = fmaf(fabsf(t0), 0.5f, 0.5f); f1 = fmaf(fabsf(t1), 0.5f, 0.5f);
     float r0 = fmaxf(z0, 0.f), r1 = fmaxf(z1, 0.f);
     if (SL) {
       const bool valid0 = j < nvalid, valid1 = j + 1 < nvalid;
@@ -76,9 +93,52 @@ __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, ui
   }
 }
 
+// The exact-enough evaluation of 32 logits (see epi32), ONE copy of the code for every caller: it is rare on a freshly
+// initialised layer, and four inlined copies per call site pushed the forward kernels out of the instruction cache
+// (0.184 -> 0.262 ms).  io: v[32] accumulators in, then R[4], P[4] in/out at 32..39 and out[16] at 40..55 (a call through
+// memory; only this path pays for it).
+static __device__ __noinline__ void epi32_wide(uint32_t* io, uint32_t sbias, int has_bias, uint32_t ymask, int nvalid, float s, float* zout) {
+  float R[4], P[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { R[k] = __uint_as_float(io[32 + k]); P[k] = __uint_as_float(io[36 + k]); }
+#pragma unroll 4
+  for (int j = 0; j < 32; j += 2) {
+    float z0 = __uint_as_float(io[j]), z1 = __uint_as_float(io[j + 1]);
+    if (has_bias) {
+      float b0, b1;
+      asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(b0), "=f"(b1) : "r"(sbias + j * 4));
+      z0 += b0; z1 += b1;
+    }
+    const float e0 = ex2_approx(fabsf(z0) * -1.4426950408889634f), e1 = ex2_approx(fabsf(z1) * -1.4426950408889634f);
+    float f0 = rcp_approx(1.f + e0), f1 = rcp_approx(1.f + e1);            // sigma(|z|)
+    float d0 = s * (z0 >= 0.f ? f0 : e0 * f0), d1 = s * (z1 >= 0.f ? f1 : e1 * f1);
+    float r0 = fmaxf(z0, 0.f), r1 = fmaxf(z1, 0.f);
+    if ((ymask >> j) & 1u) { d0 -= s; r0 -= z0; }
+    if ((ymask >> (j + 1)) & 1u) { d1 -= s; r1 -= z1; }
+    if (j >= nvalid) { d0 = 0.f; f0 = 1.f; r0 = 0.f; }
+    if (j + 1 >= nvalid) { d1 = 0.f; f1 = 1.f; r1 = 0.f; }
+    if (zout && j < nvalid) zout[j] = z0;
+    if (zout && j + 1 < nvalid) zout[j + 1] = z1;
+    // same chains as the packed code: logit jj feeds R[jj & 3] and P[jj & 3]
+    P[j & 3] *= f0; P[(j + 1) & 3] *= f1;
+    R[j & 3] += r0; R[(j + 1) & 3] += r1;
+    io[40 + (j >> 1)] = pack_bf16x2(d0, d1);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { io[32 + k] = __float_as_uint(R[k]); io[36 + k] = __float_as_uint(P[k]); }
+}
+
 // 32 logits of one batch row: z -> dY (bf16x2 packed) and the row's loss terms.
-//   sigma(z) = 1/2 + 1/2 tanh(z/2)  (one MUFU op);  softplus(z) = max(z,0) - ln( sigma(|z|) ), and the
-//   logs of a tile are taken once on the PRODUCT of the factors sigma(|z|) in [1/2,1)  (<= 16 per chain).
+//   softplus(z) = max(z,0) - ln( sigma(|z|) ), and the logs of a tile are taken once on the PRODUCT of the factors
+//   sigma(|z|) in [1/2,1]  (<= 16 per chain).
+// sigma has two evaluations:
+//   fast: sigma(z) = 1/2 + 1/2 tanh.approx(z/2), ONE MUFU op per logit.  tanh.approx is good to 2^-11 RELATIVE to tanh,
+//         i.e. up to 2.4e-4 absolute on sigma: 0.3 % of sigma(-2.5) = 0.076, the size of the bf16 rounding of dY, and
+//         worse below.  So it is accepted only if every |z| of the warp's 32 x 32 logits is <= 2.5 (bounded by
+//         max |accumulator| + max |bias|; true of a freshly initialised layer: |z| has std 0.23 in config 3's tail and
+//         0.55 in its dense head);
+//   wide: otherwise (the trained regime: confident negatives, sigma ~ 1e-4) the 32 logits are evaluated with
+//         e = 2^(-|z| log2 e), sigma(|z|) = 1/(1+e), sigma(-|z|) = e/(1+e): two MUFU ops, relative error ~1e-6 for any z.
 // SLOW: some label of this chunk may be a positive of some row of the warp, or the chunk holds padding labels (>= L), or
 // logits are wanted; the decision is then refined per 8 logits (warp-uniform), because the special-case code costs more
 // than the math itself and positives are rare (in the dense head ~70 % of the (warp, 128-label tile) pairs hold one).
@@ -86,15 +146,37 @@ __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, ui
 template <bool SLOW, bool BIAS>
 __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
                                       float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
+  // which evaluation: max |accumulator| over the warp's 32 x 32 logits (+ max |bias| of the 32 labels) against 2.5
+  float am = 0.f;
+#pragma unroll
+  for (int j = 0; j < 32; j += 2) am = max3(am, fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1])));
+  if (BIAS) {
+    float b;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(b) : "r"(sbias + (threadIdx.x & 31) * 4));
+    am += __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fabsf(b))));
+  }
+  if (__any_sync(0xffffffffu, am > 2.5f)) {
+    uint32_t io[56];
+#pragma unroll
+    for (int j = 0; j < 32; ++j) io[j] = v[j];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { io[32 + k] = __float_as_uint(R[k]); io[36 + k] = __float_as_uint(P[k]); }
+    epi32_wide(io, sbias, BIAS ? 1 : 0, SLOW ? ymask : 0u, SLOW ? nvalid : 32, s, SLOW ? zout : nullptr);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { R[k] = __uint_as_float(io[32 + k]); P[k] = __uint_as_float(io[36 + k]); }
+#pragma unroll
+    for (int k = 0; k < 16; ++k) out[k] = io[40 + k];
+    return;
+  }
   uint64_t R2[2] = {pk2(R[0], R[1]), pk2(R[2], R[3])}, P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};
   const uint64_t half2 = pk2(0.5f, 0.5f), hs2 = pk2(hs, hs);
 #define HASTE_EPI8(J0_)                                                                                             \
   if (SLOW) {                                                                                                        \
     const bool sl = __any_sync(0xffffffffu, ((ymask >> J0_) & 0xffu) != 0u) || nvalid < J0_ + 8 || zout != nullptr; \
-    if (sl) epi8<true, BIAS, J0_>(v, sbias, ymask, nvalid, s, half2, hs2, R2, P2, out, zout);                        \
-    else epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                              \
+    if (sl) epi8<true, BIAS, J0_>(v, sbias, ymask, nvalid, s, half2, hs2, R2, P2, out, zout);                  \
+    else epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                        \
   } else {                                                                                                           \
-    epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                                   \
+    epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                             \
   }
   HASTE_EPI8(0) HASTE_EPI8(8) HASTE_EPI8(16) HASTE_EPI8(24)
 #undef HASTE_EPI8

@@ -116,3 +116,28 @@ def test_head_empty():
     loss = torch.full((1,), 3.0, device=dev)
     head.forward_loss(8, torch.zeros(8, 16, device=dev), torch.zeros(1, 16, device=dev), None, None, None, loss=loss)
     assert loss.item() == 0.0
+
+
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_head_trained_regime_confident_negatives(oracle, force_simt):
+    """Same gate as tests/test_gpu_tail.py::test_trained_regime_confident_negatives for the dense head: logits in
+    [-12, -4] with a few confident positives; dY elementwise, loss by relative error."""
+    from paper_2606_01117_b200 import haste
+    B, d, Lh = 256, 256, 128 * 5 + 24
+    X, W, bias, rowptr, col, bits = _case(91, B, d, Lh, "bf16", True, w_std=0.01, L_total=Lh + 50)
+    rng = np.random.RandomState(4)
+    bias = rng.uniform(-12.0, -4.0, size=Lh).astype(np.float32)
+    bias[7::89] = 6.0
+    bias[13::83] = -1.0
+    dev = torch.device("cuda:0")
+    head = haste.HasteHead(d, Lh, B, "bf16", flags=haste.HASTE_FORCE_SIMT if force_simt else 0)
+    loss = torch.full((1,), float("nan"), device=dev)
+    dY = torch.full((B, Lh), float("nan"), dtype=head.tdtype, device=dev)
+    head.forward_loss(B, _dev(X, bits["X"]), _dev(W, bits["W"]), _dev(bias), _dev(rowptr), _dev(col), loss=loss, dY=dY)
+    ref = oracle.head_forward(X, W, bias, rowptr, col)
+    assert np.all((ref["z"] < -3.0) | (ref["z"] > -2.4))
+    assert abs(loss.item() - ref["loss"]) <= 1e-3 * abs(ref["loss"]), (loss.item(), ref["loss"])
+    dYn = dY.float().cpu().numpy()
+    rel = np.abs(dYn - ref["dY"]) / np.abs(ref["dY"])
+    assert rel.max() <= 6e-3, rel.max()
+    assert np.all(np.sign(dYn) == np.sign(ref["dY"]))

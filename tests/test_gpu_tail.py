@@ -242,3 +242,32 @@ def test_w_zero_closed_form(H):
     for i in range(B):
         Y[i, inp.col[inp.rowptr[i]:inp.rowptr[i + 1]]] = 1
     assert np.allclose(out["dY"], (0.5 - Y) / B, rtol=0, atol=1e-7)
+
+
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_trained_regime_confident_negatives(oracle, H, force_simt):
+    """The regime of a trained XMC layer: almost every logit is a confident negative (z in [-12, -4], sigma 1e-5 .. 2e-2),
+    a few labels are confident positives.  dY = s sigma(z) and the loss terms ln(1 + e^z) are then tiny numbers, and an
+    evaluation of sigma with a fixed ABSOLUTE error (1/2 + 1/2 tanh.approx: 2.4e-4) is wrong by multiples of their
+    value.  Gate: ELEMENTWISE relative error of dY (bf16 rounding 2^-9 plus the approximation), the loss by relative
+    error, and the backward from the kernel's own dY."""
+    from gpu_util import TailRun
+    B, d, L, G, K = 256, 128, 64 * 9 + 5, 64, 64
+    inp = synth.small_case(61, B, d, L, G, K, dtype="bf16", w_std=0.02, with_bias=True, n_pos=4)
+    rng = np.random.RandomState(3)
+    inp.bias = rng.uniform(-12.0, -4.0, size=L).astype(np.float32)
+    inp.bias[5::97] = 6.0                                   # a few confident positives
+    inp.bias[11::101] = -1.0                                # and some labels in the middle (both evaluations inside one group)
+    run = TailRun(inp, G, flags=(H.HASTE_FORCE_SIMT if force_simt else 0) | H.HASTE_IDX_SORTED_DISTINCT)
+    out = run.forward()
+    ref = oracle.tail_forward(inp.X, inp.idx, inp.W, inp.bias, inp.rowptr, inp.col, G)
+    assert np.all((ref["z"] < -3.0) | (ref["z"] > -2.4))
+    assert abs(out["loss"] - ref["loss"]) <= 1e-3 * abs(ref["loss"]), (out["loss"], ref["loss"])
+    rel = np.abs(out["dY"] - ref["dY"]) / np.abs(ref["dY"])
+    assert rel.max() <= 6e-3, (rel.max(), np.unravel_index(rel.argmax(), rel.shape))
+    assert np.all(np.sign(out["dY"]) == np.sign(ref["dY"]))
+    neg = ref["z"] < -3.0
+    assert oracle.rel_l2(out["dY"][neg], ref["dY"][neg]) <= 5e-3           # the confident negatives on their own
+    bout = run.backward()
+    bref = oracle.tail_backward(inp.X, inp.idx, inp.W, ref["dY"], G)
+    _check_backward(oracle, bout, bref, 5e-3, G)
