@@ -455,10 +455,7 @@ def main():
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
-    nprof = min(args.steps, 1024)      # per-kernel event ring of the library: the last nprof calls of the timed region
-    layer.set_profiling(nprof)
-    if use_head:
-        head.set_profiling(nprof)
+    # ---- the timed region of `value`: K steps through the four public calls, nothing else on the stream
     launches[0] = 0
     sampler = ClockSampler(local)
     if rank == 0 and not os.environ.get("HASTE_NO_CLOCKS"):
@@ -466,18 +463,52 @@ def main():
     ms_total = timed(step, args.steps)
     clocks = sampler.stop() if rank == 0 else None
     n_launch = launches[0]
-    # per-kernel device times of the timed region (CUDA events recorded inside the library, on the launch stream)
+    # ---- a separate pass for the per-kernel breakdown: the library records CUDA events on the launch stream around each
+    # kernel (16 records per step, ~2-5 % of the step), so these K steps are not the ones `value` is computed from
+    nprof = min(args.steps, 1024)
+    layer.set_profiling(nprof)
+    if use_head:
+        head.set_profiling(nprof)
+    ms_prof = timed(step, args.steps)
     kn = {"forward": haste.KERNEL_FORWARD, "dW": haste.KERNEL_DW, "dX": haste.KERNEL_DX,
           "prep_fwd": haste.KERNEL_PREP_FWD, "prep_bwd": haste.KERNEL_PREP_BWD, "post_bwd": haste.KERNEL_POST_BWD}
     kms = {k: [layer.kernel_ms(v, a) for a in range(nprof)] for k, v in kn.items()}
     if use_head:
         kms["head_forward"] = [head.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nprof)]
         kms["head_backward"] = [head.kernel_ms(haste.KERNEL_DW, a) for a in range(nprof)]
+    # ---- forward in logits-only mode: haste_forward_logits, no targets, no loss; the B x L logits are
+    # written in the storage dtype (library layout).  Beside it the FLOPs-matched dense bottleneck's forward
+    # [B,K] x [L,K]^T in the same dtype through cuBLAS (torch.matmul): a library comparison point, not product code.
+    logits_only = None
+    if rank == 0 and layer.kernel_family == 1:
+        nlog = min(args.steps, nprof, 50)
+        for _ in range(2):
+            layer.forward_logits(B, X, idx, W, None, dY)
+        torch.cuda.synchronize()
+        for _ in range(nlog):
+            layer.forward_logits(B, X, idx, W, None, dY)
+        torch.cuda.synchronize()
+        lms = [layer.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nlog)]
+        Lp = (L + 7) // 8 * 8                        # cuBLAS wants 16-byte rows: pad the label count of the comparison
+        Hb = torch.randn(B, K, device=dev).to(tdt)
+        Wp = torch.zeros(Lp, K, dtype=tdt, device=dev)
+        Wp[:L] = W
+        Zb = torch.empty(B, Lp, dtype=tdt, device=dev)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nlog)]
+        torch.matmul(Hb, Wp.t(), out=Zb)
+        for a, b_ in evs:
+            a.record(); torch.matmul(Hb, Wp.t(), out=Zb); b_.record()
+        torch.cuda.synchronize()
+        dms = [a.elapsed_time(b_) for a, b_ in evs]
+        lb = L * K * esz + cfg.NG * K * 4 + B * d * esz + cfg.NG * G * B * esz
+        logits_only = {"ms": float(np.mean(lms)), "ms_median": float(np.median(lms)), "ms_min": float(np.min(lms)), "alg_bytes": int(lb),
+                       "logits_dtype": cfg.dtype, "dense_bottleneck_ms": float(np.median(dms)),
+                       "dense_bottleneck_note": "torch.matmul [B,%d] x [L,%d]^T -> [B,L] in %s (cuBLAS), same FLOPs and W/output bytes, no gather" % (K, K, cfg.dtype)}
+        del Zb, Hb, Wp
+        layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY)     # dY holds dY again for what follows
     layer.set_profiling(0)
     if use_head:
         head.set_profiling(0)
-    # the same K steps once more with the library's per-kernel events off: what the instrumentation of the timed region costs
-    ms_plain = timed(step, args.steps)
     for _ in range(2):
         step_e2e()
     ms_e2e = timed(step_e2e, args.steps, finish_e2e)
@@ -497,31 +528,45 @@ def main():
     value = whole_job_tflops(world, step_flops, ms_step)
     e2e_value = whole_job_tflops(world, step_flops, ms_e2e / args.steps)
     ab = _alg_bytes(cfg)
+    SPEC_HBM, SPEC_BF16 = 8000.0, 2250.0          # B200 nominal: HBM3e GB/s, dense bf16 TFLOP/s
     kernels = {}
     for k in ("forward", "dW", "dX"):
-        mean = float(np.mean(kms[k]))
+        mean, med = float(np.mean(kms[k])), float(np.median(kms[k]))
         gbs = ab[k] / (mean * 1e-3) / 1e9
-        kernels[k] = {"ms": mean, "ms_min": float(np.min(kms[k])), "GB/s": gbs, "frac_hbm": gbs / peaks["hbm"],
-                      "TFLOP/s": tail_f / (mean * 1e-3) / 1e12, "alg_bytes": ab[k]}
+        kernels[k] = {"ms": mean, "ms_median": med, "ms_min": float(np.min(kms[k])), "GB/s": gbs, "frac_hbm": gbs / peaks["hbm"],
+                      "frac_hbm_spec": gbs / SPEC_HBM, "TFLOP/s": tail_f / (mean * 1e-3) / 1e12, "alg_bytes": ab[k]}
     for k in kms:
         if k not in kernels:
-            kernels[k] = {"ms": float(np.mean(kms[k])), "ms_min": float(np.min(kms[k]))}
+            kernels[k] = {"ms": float(np.mean(kms[k])), "ms_median": float(np.median(kms[k])), "ms_min": float(np.min(kms[k]))}
     if use_head:
-        kernels["head_forward"]["TFLOP/s"] = head_f / (kernels["head_forward"]["ms"] * 1e-3) / 1e12
-        kernels["head_backward"]["TFLOP/s"] = 2 * head_f / (kernels["head_backward"]["ms"] * 1e-3) / 1e12
+        for k, fl in (("head_forward", head_f), ("head_backward", 2 * head_f)):
+            tf = fl / (kernels[k]["ms"] * 1e-3) / 1e12
+            kernels[k].update({"TFLOP/s": tf, "frac_tensor": tf / peaks["bf16_sustained"], "frac_tensor_burst": tf / peaks["bf16"],
+                               "frac_tensor_spec": tf / SPEC_BF16})
+    if logits_only is not None:
+        g = logits_only["alg_bytes"] / (logits_only["ms"] * 1e-3) / 1e9
+        logits_only.update({"GB/s": g, "frac_hbm": g / peaks["hbm"], "frac_hbm_spec": g / SPEC_HBM})
+        kernels["forward_logits_only"] = logits_only
     dom = max(("forward", "dW", "dX"), key=lambda k: kernels[k]["ms"])
-    # DRAM bytes per launch of that kernel from the committed ncu --set full capture (profiles/r01_ncu_traffic.txt); null for other workloads
-    traffic = None
+    # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture of this round.  The record names the
+    # kernel and carries the SHA-256 of the kernel source it was captured from: a stale record (source changed since) gives null.
+    traffic, traffic_src = None, None
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_ncu_traffic.txt")))
-        if tj.get("workload") == args.workload:
-            traffic = tj.get(dom)
+        import hashlib
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r02_ncu_traffic.txt")))
+        rec = tj.get(dom) if tj.get("workload") == args.workload else None
+        if rec:
+            h = hashlib.sha256(open(os.path.join(ROOT, rec["source"]), "rb").read()).hexdigest()
+            if h == rec["source_sha256"]:
+                traffic, traffic_src = rec["dram_bytes"], {"kernel": rec["kernel"], "capture": rec["capture"], "source": rec["source"]}
     except Exception:
         traffic = None
     roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["GB/s"], "peak": peaks["hbm"], "unit": "GB/s",
-                "frac": kernels[dom]["GB/s"] / peaks["hbm"], "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)",
+                "frac": kernels[dom]["GB/s"] / peaks["hbm"], "frac_spec": kernels[dom]["GB/s"] / SPEC_HBM, "peak_spec": SPEC_HBM,
+                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write)", "traffic_from": traffic_src,
                 "algorithmic_bytes": ab[dom], "peak_source": peaks["source"] + " (burst copy)",
-                "share_of_step": kernels[dom]["ms"] / ms_step}
+                "share_of_step": kernels[dom]["ms"] / (ms_prof / args.steps),
+                "timing": "CUDA events on the launch stream around the kernel, mean over the K steps of a separate profiled pass"}
     pass_mb = (L * K * esz >> 20, cfg.NG * G * B * esz >> 20)
     if sum(pass_mb) > 126:
         l2_note = "inputs larger than L2 (per pass W %d MB + dY %d MB vs 126 MB L2); no explicit flush" % pass_mb
@@ -537,10 +582,10 @@ def main():
                    "G": G, "K": K, "replicas": world, "l2": l2_note,
                    "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}, "deterministic": bool(args.deterministic)},
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "note": "copies on their own streams, two sets of device buffers; no per-kernel events in this run (compare with events_off)"},
+                "note": "copies on their own streams, two sets of device buffers; no per-kernel events"},
         "gpu_launches": int(n_launch), "clocks": clocks, "roofline": roofline, "kernels": kernels,
-        "events_off": {"ms_per_step": ms_plain / args.steps, "value": whole_job_tflops(world, step_flops, ms_plain / args.steps),
-                       "note": "same K steps repeated without the per-kernel CUDA events that the timed region carries"},
+        "profiled_pass": {"ms_per_step": ms_prof / args.steps,
+                          "note": "the same K steps repeated with the library's per-kernel CUDA events on; `kernels` and `roofline` come from this pass, `value` does not"},
         "loss": [float(v) for v in loss.cpu().tolist()],
     }
     if not args.no_cpu_baseline and world == 1:

@@ -112,6 +112,14 @@ int haste_forward_loss(haste_layer_t* h, int B,
                        float* logits_out,         /* optional [B,L] row-major fp32, or NULL                   */
                        void* stream);
 
+/* Logits-only forward (z = <w_l, h_I> per label; the inference pass behind Eq. 4):
+ * Z receives z[i,l] = bias[l] + sum_j W[l,j] X[i, idx[l/G, j]] rounded to `dtype`, in the library's dY layout
+ * ([NG][B][G], haste_dy_bytes(h,B) bytes, padding labels >= L written as zero; haste_dy_unpack converts it to
+ * [B,L] fp32).  No targets, no loss, nothing else written.  tcgen05 kernel family only (HASTE_ERR_UNSUPPORTED
+ * otherwise: use haste_forward_loss with logits_out there).  X, idx, W, Z 16-byte aligned. */
+int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W,
+                         const float* bias /* [L] fp32 or NULL */, void* Z, void* stream);
+
 /* Backward from a dY in the library layout. */
 int haste_backward(haste_layer_t* h, int B,
                    const void* X, const int32_t* idx, const void* W, const void* dY,

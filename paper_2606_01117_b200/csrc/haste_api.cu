@@ -291,7 +291,7 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
     int n = 0;
     pf.begin(HASTE_KERNEL_FORWARD, st);
     rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY,
-                         logits_out, st, &n);
+                         logits_out, 0, st, &n);
     if (rc) return rc;
     pf.end(HASTE_KERNEL_FORWARD, st);
     h->last_launches += n;
@@ -314,6 +314,39 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
     if (rc) return rc;
     h->last_launches++;
   }
+  return HASTE_OK;
+}
+
+int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias, void* Z,
+                         void* stream) {
+  int rc = check_call(h, B, "haste_forward_logits");
+  if (rc) return rc;
+  if (!X || !idx || !W || !Z) { set_error("haste_forward_logits: X, idx, W and Z are required"); return HASTE_ERR_INVALID_ARG; }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(Z) || !aligned16(idx)) {
+    set_error("haste_forward_logits: X, W, idx and Z must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (h->family != 1) {
+    set_error("haste_forward_logits: only the tcgen05 kernel family has a logits-only forward (use haste_forward_loss with logits_out)");
+    return HASTE_ERR_UNSUPPORTED;
+  }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const TailShape sh = make_shape(h, B);
+  Profiler& pf = *h->prof;
+  h->last_launches = 0;
+  if (B == 0 || h->NG == 0) return HASTE_OK;
+  pf.begin(HASTE_KERNEL_PREP_FWD, st);
+  rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+  if (rc) return rc;
+  h->last_launches++;
+  pf.end(HASTE_KERNEL_PREP_FWD, st);
+  int n = 0;
+  pf.begin(HASTE_KERNEL_FORWARD, st);
+  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, Z, nullptr, 1, st, &n);
+  if (rc) return rc;
+  pf.end(HASTE_KERNEL_FORWARD, st);
+  h->last_launches += n;
   return HASTE_OK;
 }
 

@@ -15,9 +15,10 @@ int tc_tail_create(TcTailState** out, const haste_config_t& cfg, int Bpad, int d
 void tc_tail_destroy(TcTailState* s);
 int tc_tail_num_partials(const TcTailState* s);
 // loss_partials: per-CTA unscaled loss partials [tc_tail_num_partials] or NULL.
+// z_mode = 1: logits-only forward, the dY buffer receives the logits (same layout and dtype); no targets, no loss.
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
                     const float* bias, const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY,
-                    float* logits_out, cudaStream_t st, int* n_launches);
+                    float* logits_out, int z_mode, cudaStream_t st, int* n_launches);
 int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
                float* dbias, cudaStream_t st, int* n_launches);
 // dx_part: null, or (HASTE_DETERMINISTIC) private partial tiles [tc_tail_dx_parts()][d][128] fp32, zeroed by the caller: the kernel

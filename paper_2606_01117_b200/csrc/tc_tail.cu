@@ -71,6 +71,7 @@ struct FwdParams {
   float* partials;         // [gridDim.x] unscaled loss partials, or null
   float* logits;           // [B][L] fp32 or null
   int write_dy;
+  int z_mode;              // 1: the dY buffer receives the logits themselves (bf16, same layout); no targets, no loss
   int B, Bpad, NT, NP, S;  // NT batch tiles of 128; NP tile pairs; S group stripes (grid = NP*S)
   int64_t L, NG, label_offset;
   float s;
@@ -307,7 +308,18 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         float* zout = (p.logits && valid_row) ? p.logits + (size_t)b * p.L + g * G + sc * 32 : nullptr;
         const int nvalid = nl - sc * 32;
         const uint32_t sb = sbias_w + sc * 128;
-        if (slow) {
+        if (p.z_mode) {           // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
+#pragma unroll
+          for (int j = 0; j < 32; j += 2) {
+            float z0 = __uint_as_float(v[j]), z1 = __uint_as_float(v[j + 1]);
+            if (p.bias) {
+              float b0, b1;
+              asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(b0), "=f"(b1) : "r"(sb + j * 4));
+              z0 += b0; z1 += b1;
+            }
+            out[j >> 1] = pack_bf16x2(j < nvalid ? z0 : 0.f, j + 1 < nvalid ? z1 : 0.f);
+          }
+        } else if (slow) {
           if (p.bias) epi32<true, true>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
           else epi32<true, false>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
         } else {
@@ -389,7 +401,7 @@ int tc_tail_num_partials(const TcTailState* s) { return s->n_partials; }
 
 template <int G, int K>
 static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
-                      const int32_t* rowptr, const int32_t* col, float* partials, void* dY, float* logits, cudaStream_t st) {
+                      const int32_t* rowptr, const int32_t* col, float* partials, void* dY, float* logits, int z_mode, cudaStream_t st) {
   using C = FwdCfg<G, K>;
   static_assert(C::SMEM <= 232448, "shared memory budget");
   CUtensorMap tmW, tmY;
@@ -412,6 +424,7 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   FwdParams p;
   p.Xt = (const bf16*)Xt; p.idx = idx; p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = partials; p.logits = logits;
   p.write_dy = dY ? 1 : 0;
+  p.z_mode = z_mode;
   p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NP = (p.NT + 1) / 2;
   p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NP));
   p.L = sh.L; p.NG = sh.NG; p.label_offset = sh.label_offset; p.s = sh.s;
@@ -427,10 +440,10 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
 
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
                     const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
-                    cudaStream_t st, int* n_launches) {
+                    int z_mode, cudaStream_t st, int* n_launches) {
   *n_launches = 1;
 #define HASTE_FWD(G_, K_) \
-  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, dY, logits_out, st)
+  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, dY, logits_out, z_mode, st)
   HASTE_FWD(64, 128); HASTE_FWD(64, 64); HASTE_FWD(32, 64); HASTE_FWD(32, 128); HASTE_FWD(128, 64); HASTE_FWD(128, 128);
 #undef HASTE_FWD
   set_error("tcgen05 forward: unsupported (G, K)");

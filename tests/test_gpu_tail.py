@@ -271,3 +271,29 @@ def test_trained_regime_confident_negatives(oracle, H, force_simt):
     bout = run.backward()
     bref = oracle.tail_backward(inp.X, inp.idx, inp.W, ref["dY"], G)
     _check_backward(oracle, bout, bref, 5e-3, G)
+
+
+@pytest.mark.parametrize("shape", [(300, 768, 64 * 23 + 11, 64, 128), (130, 256, 32 * 9 + 5, 32, 64), (64, 512, 128 * 5 + 3, 128, 128)])
+@pytest.mark.parametrize("with_bias", [False, True])
+def test_forward_logits_only(oracle, H, shape, with_bias):
+    """haste_forward_logits: z = bias + sum_j W[l,j] X[i, idx[l/G, j]] rounded once to bf16, in the library
+    layout; padding labels of the last group are written as zero; nothing else is needed (no targets)."""
+    from gpu_util import TailRun
+    B, d, L, G, K = shape
+    inp = synth.small_case(70 + B, B, d, L, G, K, dtype="bf16", with_bias=with_bias, w_std=0.2)
+    run = TailRun(inp, G, want_logits=False)
+    assert run.layer.kernel_family == 1
+    Z = run.layer.alloc_dy(B)
+    Z.fill_(float("nan"))
+    run.layer.forward_logits(B, run.X, run.idx, run.W, run.bias, Z)
+    zf = torch.empty(B, L, device=Z.device)
+    run.layer.dy_unpack(B, Z, zf)
+    ref = oracle.tail_forward(inp.X, inp.idx, inp.W, inp.bias, inp.rowptr, inp.col, G)["z"]
+    want = synth.round_bf16(ref.astype(np.float32))[1].reshape(B, L)          # the fp64 logits rounded once to bf16
+    got = zf.cpu().numpy()
+    # fp32 accumulation before the rounding can move a value across a bf16 rounding boundary: allow one bf16 step there
+    assert np.max(np.abs(got - want) / np.maximum(np.abs(want), 1e-3)) <= 2.0 ** -7
+    assert oracle.rel_l2(got, ref) <= 3e-3
+    NG = -(-L // G)
+    if NG * G > L:
+        assert torch.count_nonzero(Z.view(NG, B, G)[NG - 1, :, L - (NG - 1) * G:]).item() == 0
