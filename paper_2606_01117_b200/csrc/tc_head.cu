@@ -348,6 +348,218 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Forward with 256 x 256 output tiles (two M = 128 accumulators of N = 256: all 512 TMEM columns), for batches of more
+// than 128 rows.  Why: with 128 x 128 tiles the kernel is bound by its operand traffic through L2 (201 MB at config 3,
+// 23 of its 27 us) and by 3.46 waves of tiles on 148 SMs.  A 256 x 256 tile moves 64 KB per k-block for four times the
+// MMA work (98 MB in all), config 3 becomes ONE wave of 128 tiles, and the MMA phase of a tile (96 MMAs of 128 cycles)
+// is as long as its loads.  There is one accumulator set, so a CTA's epilogue does not overlap its next tile's MMAs: with
+// one tile per CTA nothing is lost.  The CSR scan of the thread's two rows runs before the accumulators are waited for.
+// warp roles (576 threads): warps 0-15 epilogue (warp w: TMEM lane quadrant w & 3, M tile (w >> 2) & 1, 128-label half
+// w >> 3; four per scheduler, because one warp's chunk is a latency chain: 8 warps took 14.8 k cycles, the MMA phase 16 k),
+// warp 16 MMA, warp 17 TMA.
+// ---------------------------------------------------------------------------------------------
+struct Fwd256Cfg {
+  static constexpr int BN = 256, NST = 3;
+  static constexpr int A_BYTES = 32768, B_BYTES = 32768, STAGE = A_BYTES + B_BYTES;
+  static constexpr int NEW = 16;                            // epilogue warps
+  static constexpr int OFF_EPI = 0;                         // [16 warps][2 buffers][32 rows][128 B] OVER the operand stages: a
+                                                            // tile's epilogue starts when its last MMA has read them, and the
+                                                            // loader waits for the epilogue before it loads the next tile
+  static constexpr int OFF_BIAS = NST * STAGE;              // [256] fp32, one copy per CTA
+  static constexpr int OFF_BAR = OFF_BIAS + 1024;
+  static constexpr int OFF_MISC = OFF_BAR + (2 * NST + 2) * 8;
+  static constexpr int SMEM = OFF_MISC + 128 + 1024;
+  static constexpr int THREADS = (NEW + 2) * 32;
+};
+
+__global__ void __launch_bounds__(Fwd256Cfg::THREADS, 1)
+tc_head_fwd256_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                      const __grid_constant__ CUtensorMap tmO, const HeadParams p) {
+  using C = Fwd256Cfg;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t sbase = smem_u32(smem);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
+  uint64_t* full = bars;                    // [NST] count 1 + tx
+  uint64_t* empty = bars + C::NST;          // [NST] count 1 (umma commit)
+  uint64_t* t_full = bars + 2 * C::NST;     // count 1
+  uint64_t* t_empty = t_full + 1;           // count 16: accumulators AND staging (= operand stages) free again
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
+  float* loss_red = reinterpret_cast<float*>(smem + C::OFF_MISC + 16);   // [16]
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_items = p.MT * p.NTL;         // MT = tiles of 256 rows, NTL = tiles of 256 labels
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
+    mbar_init(t_full, 1); mbar_init(t_empty, C::NEW);
+    fence_barrier_init();
+  }
+  if (warp == C::NEW + 1 && lane == 0) { tma_prefetch_desc(&tmA); tma_prefetch_desc(&tmB); tma_prefetch_desc(&tmO); }
+  if (warp == C::NEW) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == C::NEW + 1) {
+    if (lane == 0) {
+      int it = 0, n = 0;
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++n) {
+        const int mt = w % p.MT, nt = w / p.MT;
+        mbar_wait(t_empty, (n & 1) ^ 1);       // the previous tile's epilogue has left the staging rows (they overlay the stages)
+        for (int kb = 0; kb < p.KB; ++kb, ++it) {
+          const int st = it % C::NST;
+          mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
+          mbar_arrive_expect_tx(&full[st], C::STAGE);
+          uint8_t* a = smem + st * C::STAGE;
+          tma_load_2d(a, &tmA, &full[st], kb * 64, mt * 256);                    // box {64, 256}: both M tiles
+          tma_load_2d(a + C::A_BYTES, &tmB, &full[st], kb * 64, nt * 256);       // box {64, 256}
+        }
+      }
+    }
+  } else if (warp == C::NEW) {
+    constexpr uint32_t idesc = make_idesc_bf16(128, 256, 0, 0);
+    const uint64_t adesc0 = make_sdesc_sw128(sbase, 16, 1024);
+    const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::A_BYTES, 16, 1024);
+    int it = 0, n = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++n) {
+      mbar_wait(t_empty, (n & 1) ^ 1);
+      tc_fence_after();
+      for (int kb = 0; kb < p.KB; ++kb, ++it) {
+        const int st = it % C::NST;
+        mbar_wait(&full[st], (it / C::NST) & 1);
+        tc_fence_after();
+        if (elect_one()) {
+          const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const uint32_t acc = (kb > 0 || j > 0) ? 1u : 0u;
+            const uint64_t bd = bdesc0 + so + (uint64_t)((j * 32) >> 4);
+            umma_f16(tmem_base, adesc0 + so + (uint64_t)((j * 32) >> 4), bd, idesc, acc);
+            umma_f16(tmem_base + 256, adesc0 + so + (uint64_t)((16384 + j * 32) >> 4), bd, idesc, acc);
+          }
+          umma_commit(&empty[st]);
+          if (kb == p.KB - 1) umma_commit(t_full);
+        }
+        __syncwarp();
+      }
+    }
+  } else {
+    const int q = warp & 3, tile = (warp >> 2) & 1, half = warp >> 3;
+    const uint32_t swz = (uint32_t)(lane & 7);
+    const uint32_t sbuf0 = sbase + C::OFF_EPI + warp * 8192;
+    uint8_t* sbuf0_ptr = smem + C::OFF_EPI + warp * 8192;
+    int nstore = 0;
+    const uint32_t sbias = sbase + C::OFF_BIAS;
+    const float hs = 0.5f * p.s;
+    float loss_local = 0.f;
+    int n = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++n) {
+      const int mt = w % p.MT, nt = w / p.MT;
+      const int row = mt * 256 + tile * 128 + q * 32 + lane;
+      const int n0 = nt * 256;
+      const bool valid_row = row < p.B;
+      const int nl = (int)min((int64_t)256, p.L - n0);
+      // positives of this row inside the tile's 256 labels: binary search for the first column >= n0, then walk
+      uint32_t ym[4] = {0u, 0u, 0u, 0u};          // this warp's four 32-label chunks: labels n0 + half * 128 ...
+      if (valid_row && p.rowptr) {
+        int lo = __ldg(p.rowptr + row);
+        const int pe = __ldg(p.rowptr + row + 1);
+        int hi = pe;
+        const int64_t want = (int64_t)n0 + half * 128 + p.label_offset;
+        while (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if ((int64_t)__ldg(p.col + mid) < want) lo = mid + 1; else hi = mid;
+        }
+        for (int pc = lo; pc < pe; ++pc) {
+          const int64_t o = (int64_t)__ldg(p.col + pc) - want;
+          if (o >= min(128, nl - half * 128)) break;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) if ((int)(o >> 5) == i) ym[i] |= 1u << (o & 31);
+        }
+      }
+      uint32_t anyy = ym[0] | ym[1] | ym[2] | ym[3];
+      const bool slow = __any_sync(0xffffffffu, anyy != 0) || nl < 256 || p.logits != nullptr;
+      if (p.bias) {           // one copy per CTA: epilogue warps 0-7 fill 32 labels each, then all meet at a named barrier
+        const int l = warp * 32 + lane;
+        if (warp < 8) sts32(sbias + l * 4, __float_as_uint(l < nl ? __ldg(p.bias + n0 + l) : 0.f));
+        named_bar_sync(1, C::NEW * 32);
+      }
+      mbar_wait(t_full, n & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + tile * 256 + half * 128;
+      const int nlh = nl - half * 128;                  // valid labels of this warp's half (may be <= 0)
+      float R[4] = {0.f, 0.f, 0.f, 0.f}, P[4] = {1.f, 1.f, 1.f, 1.f};
+      float lt = 0.f;
+#pragma unroll 1                 // one copy of the epilogue code (instruction cache)
+      for (int sc = 0; sc < 4; ++sc) {
+        uint32_t v[32];
+        const uint32_t ymsc = sc == 0 ? ym[0] : sc == 1 ? ym[1] : sc == 2 ? ym[2] : ym[3];
+        tmem_ld32(taddr + sc * 32, v);
+        tmem_ld_wait();
+        uint32_t out[16];
+        float* zout = (p.logits && valid_row) ? p.logits + (size_t)row * p.L + n0 + half * 128 + sc * 32 : nullptr;
+        const uint32_t sb = sbias + half * 512 + sc * 128;
+        if (slow) {
+          if (p.bias) epi32<true, true>(v, sb, ymsc, nlh - sc * 32, p.s, hs, R, P, out, zout);
+          else epi32<true, false>(v, sb, ymsc, nlh - sc * 32, p.s, hs, R, P, out, zout);
+        } else {
+          if (p.bias) epi32<false, true>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
+          else epi32<false, false>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
+        }
+        if (sc & 1) {
+          lt += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { R[i] = 0.f; P[i] = 1.f; }
+        }
+        if (p.write_out) {
+          const uint32_t sbuf = sbuf0 + (nstore & 1) * 4096;     // two staging buffers: one TMA store may still be reading
+          if ((sc & 1) == 0) {
+            if (lane == 0) bulk_wait_read<1>();
+            __syncwarp();
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const uint32_t ch = (uint32_t)((sc & 1) * 4 + i) ^ swz;
+            sts128(sbuf + lane * 128 + ch * 16, out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
+          }
+          if (sc & 1) {
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_2d(&tmO, sbuf0_ptr + (nstore & 1) * 4096, n0 + half * 128 + (sc >> 1) * 64, mt * 256 + tile * 128 + q * 32);
+              bulk_commit();
+            }
+            ++nstore;
+          }
+        }
+      }
+      if (valid_row) loss_local += lt;
+      if (lane == 0) bulk_wait_read<0>();      // this warp's TMA stores have read the staging rows: the loader may overwrite them
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(t_empty);
+      if (p.bias) named_bar_sync(1, C::NEW * 32);      // the bias copy is not refilled before every warp has used it
+    }
+    if (lane == 0) bulk_wait<0>();
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) loss_local += __shfl_xor_sync(0xffffffffu, loss_local, o);
+    if (lane == 0) loss_red[warp] = loss_local;
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == C::NEW) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
+  if (threadIdx.x == 0 && p.partials) {
+    float t = 0.f;
+#pragma unroll
+    for (int i = 0; i < C::NEW; ++i) t += loss_red[i];
+    p.partials[blockIdx.x] = t;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 struct TcHeadState {
@@ -407,6 +619,23 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
                     cudaStream_t st, int* n_launches) {
   *n_launches = 1;
   CUtensorMap tmA, tmB, tmO;
+  if (sh.B > 128) {     // 256 x 256 tiles (tc_head_fwd256_kernel)
+    int rc = map2d(&tmA, 2, X, sh.d, sh.B, 64, 256);
+    if (!rc) rc = map2d(&tmB, 2, Wh, sh.d, sh.L, 64, 256);
+    if (!rc) { if (dY) rc = map2d(&tmO, 2, dY, sh.L, sh.B, 64, 32); else tmO = tmA; }
+    if (rc) return rc;
+    HeadParams p = base_params(sh);
+    p.MT = ceil_div(sh.B, 256); p.NTL = ceil_div(sh.L, 256); p.KB = ceil_div(sh.d, 64);
+    p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = loss_partials; p.logits = logits_out; p.write_out = dY ? 1 : 0;
+    const int grid = std::min(p.MT * p.NTL, s->num_sms);
+    if (loss_partials && grid < s->n_partials)
+      HASTE_CUDA_TRY(cudaMemsetAsync(loss_partials + grid, 0, (size_t)(s->n_partials - grid) * sizeof(float), st));
+    static_assert(Fwd256Cfg::SMEM <= 232448, "shared memory budget");
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_head_fwd256_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Fwd256Cfg::SMEM));
+    tc_head_fwd256_kernel<<<grid, Fwd256Cfg::THREADS, Fwd256Cfg::SMEM, st>>>(tmA, tmB, tmO, p);
+    HASTE_LAUNCH_CHECK();
+    return HASTE_OK;
+  }
   int rc = map2d(&tmA, 2, X, sh.d, sh.B, 64, 128);
   if (!rc) rc = map2d(&tmB, 2, Wh, sh.d, sh.L, 64, 128);
   if (!rc) { if (dY) rc = map2d(&tmO, 2, dY, sh.L, sh.B, 64, 32); else tmO = tmA; }
