@@ -360,7 +360,7 @@ def main():
     X, rowptr, col = hX.to(dev), hrow.to(dev), hcol.to(dev)
     W, idx = host("W").to(dev), torch.from_numpy(inp.idx).to(dev)
     det = haste.HASTE_DETERMINISTIC if args.deterministic else 0
-    layer = haste.HasteLayer(d, L, G, K, B, cfg.dtype, label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT | det, device=local)
+    layer = haste.HasteLayer(d, L, G, K, B, cfg.dtype, label_offset=Lh, flags=haste.HASTE_IDX_SORTED_DISTINCT | haste.HASTE_XT_FROM_FORWARD | det, device=local)
     layer.validate_index(idx)
     dY = layer.alloc_dy(B)
     dW = torch.empty(L, K, dtype=tdt, device=dev)

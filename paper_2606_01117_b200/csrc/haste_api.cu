@@ -290,16 +290,11 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
   if (h->family == 1) {
     int n = 0;
     pf.begin(HASTE_KERNEL_FORWARD, st);
-    rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY,
-                         logits_out, 0, st, &n);
+    rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, loss, dY,
+                         logits_out, 0, st, &n);       // the kernel's last CTA writes the loss
     if (rc) return rc;
     pf.end(HASTE_KERNEL_FORWARD, st);
     h->last_launches += n;
-    if (loss) {
-      rc = launch_finalize_loss(nullptr, h->partials, tc_tail_num_partials(h->tc), sh.s, loss, st);
-      if (rc) return rc;
-      h->last_launches++;
-    }
     return HASTE_OK;
   }
   if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(h->loss_acc, 0, sizeof(double), st));
@@ -343,7 +338,7 @@ int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* 
   pf.end(HASTE_KERNEL_PREP_FWD, st);
   int n = 0;
   pf.begin(HASTE_KERNEL_FORWARD, st);
-  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, Z, nullptr, 1, st, &n);
+  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, nullptr, Z, nullptr, 1, st, &n);
   if (rc) return rc;
   pf.end(HASTE_KERNEL_FORWARD, st);
   h->last_launches += n;
@@ -371,9 +366,10 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
     if (dX && !accumulate_dX && B > 0) HASTE_CUDA_TRY(cudaMemsetAsync(dX, 0, (size_t)B * sh.d * 4, st));
     return HASTE_OK;
   }
-  // The gather operand X^T is rebuilt here: backward must not depend on which forward ran last.
+  // The gather operand X^T is rebuilt here: backward must not depend on which forward ran last -- unless the caller
+  // promised that it is the forward of the same step (HASTE_XT_FROM_FORWARD).
   pf.begin(HASTE_KERNEL_PREP_BWD, st);
-  if (dW || dbias) {
+  if ((dW || dbias) && !(h->cfg.flags & HASTE_XT_FROM_FORWARD)) {
     rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
     if (rc) return rc;
     h->last_launches++;
@@ -546,15 +542,10 @@ int haste_head_forward_loss(haste_head_t* h, int B, const void* X, const void* W
   if (h->family == 1) {
     int n = 0;
     pf.begin(HASTE_KERNEL_FORWARD, st);
-    rc = tc_head_forward(h->tc, sh, X, Wh, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, dY, logits_out, st, &n);
+    rc = tc_head_forward(h->tc, sh, X, Wh, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, loss, dY, logits_out, st, &n);
     if (rc) return rc;
     pf.end(HASTE_KERNEL_FORWARD, st);
     h->last_launches += n;
-    if (loss) {
-      rc = launch_finalize_loss(nullptr, h->partials, tc_head_num_partials(h->tc), sh.s, loss, st);
-      if (rc) return rc;
-      h->last_launches++;
-    }
     return HASTE_OK;
   }
   if (loss) HASTE_CUDA_TRY(cudaMemsetAsync(h->loss_acc, 0, sizeof(double), st));

@@ -196,6 +196,32 @@ __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, int a_mn_ma
          ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
+// ---------------------------------------------------------------- loss reduction across CTAs without a second launch
+// Every thread of the CTA calls this at the end of a forward kernel; `mine` is the CTA's unscaled loss partial (read from
+// thread 0).  Thread 0 publishes it and takes a ticket; the CTA that draws the last ticket sums all gridDim.x partials in
+// a FIXED order (lane i takes entries i, i+32, ...; then a fixed shuffle tree) -- the same answer whatever CTA is last --
+// writes loss = scale * sum and resets the ticket for the next call.  partials: [>= gridDim.x] floats; the ticket is the
+// word at partials[LOSS_TICKET_SLOT] (the handle allocates 1024 floats, zeroed at create).
+constexpr int LOSS_TICKET_SLOT = 1020;
+__device__ __forceinline__ void finalize_loss_last_cta(float* partials, float mine, float scale, float* loss) {
+  __shared__ int s_last;
+  unsigned* ticket = reinterpret_cast<unsigned*>(partials + LOSS_TICKET_SLOT);
+  if (threadIdx.x == 0) {
+    partials[blockIdx.x] = mine;
+    __threadfence();
+    s_last = atomicAdd(ticket, 1u) == gridDim.x - 1 ? 1 : 0;
+  }
+  __syncthreads();
+  if (s_last && threadIdx.x < 32) {
+    __threadfence();
+    double v = 0.0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += 32) v += (double)__ldcg(partials + i);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (threadIdx.x == 0) { *loss = (float)((double)scale * v); *ticket = 0u; }
+  }
+}
+
 }  // namespace tc
 
 // ---------------------------------------------------------------- host: tensor maps

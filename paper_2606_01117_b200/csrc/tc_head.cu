@@ -29,7 +29,8 @@ struct HeadParams {
   const float* bias;
   const int32_t* rowptr;
   const int32_t* col;
-  float* partials;            // FWD: per-CTA unscaled loss partials or null
+  float* partials;            // FWD: [1024] per-CTA unscaled loss partials + ticket (finalize_loss_last_cta), or null
+  float* loss;                // FWD: device scalar, written by the last CTA
   float* logits;              // FWD: [B][L] fp32 or null
   float* dbias;               // DW: [L] or null
   int write_out;              // FWD: dY; DW: dW_h
@@ -343,8 +344,8 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   tc_fence_before();
   __syncthreads();
   if (warp == 4) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
-  if (MODE == HEAD_FWD && threadIdx.x == 0 && p.partials)
-    p.partials[blockIdx.x] = (loss_red[0] + loss_red[1]) + (loss_red[2] + loss_red[3]);
+  if (MODE == HEAD_FWD && p.partials)
+    finalize_loss_last_cta(p.partials, threadIdx.x == 0 ? (loss_red[0] + loss_red[1]) + (loss_red[2] + loss_red[3]) : 0.f, p.s, p.loss);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -551,11 +552,13 @@ tc_head_fwd256_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_cons
   tc_fence_before();
   __syncthreads();
   if (warp == C::NEW) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
-  if (threadIdx.x == 0 && p.partials) {
+  if (p.partials) {
     float t = 0.f;
+    if (threadIdx.x == 0) {
 #pragma unroll
-    for (int i = 0; i < C::NEW; ++i) t += loss_red[i];
-    p.partials[blockIdx.x] = t;
+      for (int i = 0; i < C::NEW; ++i) t += loss_red[i];
+    }
+    finalize_loss_last_cta(p.partials, t, p.s, p.loss);
   }
 }
 
@@ -615,7 +618,7 @@ static HeadParams base_params(const HeadShape& sh) {
 }
 
 int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const float* bias,
-                    const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
+                    const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY, float* logits_out,
                     cudaStream_t st, int* n_launches) {
   *n_launches = 1;
   CUtensorMap tmA, tmB, tmO;
@@ -626,10 +629,8 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
     if (rc) return rc;
     HeadParams p = base_params(sh);
     p.MT = ceil_div(sh.B, 256); p.NTL = ceil_div(sh.L, 256); p.KB = ceil_div(sh.d, 64);
-    p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = loss_partials; p.logits = logits_out; p.write_out = dY ? 1 : 0;
+    p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = loss_partials; p.loss = loss; p.logits = logits_out; p.write_out = dY ? 1 : 0;
     const int grid = std::min(p.MT * p.NTL, s->num_sms);
-    if (loss_partials && grid < s->n_partials)
-      HASTE_CUDA_TRY(cudaMemsetAsync(loss_partials + grid, 0, (size_t)(s->n_partials - grid) * sizeof(float), st));
     static_assert(Fwd256Cfg::SMEM <= 232448, "shared memory budget");
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_head_fwd256_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Fwd256Cfg::SMEM));
     tc_head_fwd256_kernel<<<grid, Fwd256Cfg::THREADS, Fwd256Cfg::SMEM, st>>>(tmA, tmB, tmO, p);
@@ -642,10 +643,7 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
   if (rc) return rc;
   HeadParams p = base_params(sh);
   p.MT = ceil_div(sh.B, 128); p.NTL = ceil_div(sh.L, HeadCfg<HEAD_FWD>::BN); p.KB = ceil_div(sh.d, 64);
-  p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = loss_partials; p.logits = logits_out; p.write_out = dY ? 1 : 0;
-  const int grid = std::min(p.MT * p.NTL, s->num_sms);
-  if (loss_partials && grid < s->n_partials)
-    HASTE_CUDA_TRY(cudaMemsetAsync(loss_partials + grid, 0, (size_t)(s->n_partials - grid) * sizeof(float), st));
+  p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = loss_partials; p.loss = loss; p.logits = logits_out; p.write_out = dY ? 1 : 0;
   return launch_head<HEAD_FWD>(s, tmA, tmB, tmO, p, st);
 }
 

@@ -14,10 +14,11 @@ bool tc_tail_supported(const haste_config_t& cfg, int device);
 int tc_tail_create(TcTailState** out, const haste_config_t& cfg, int Bpad, int device);
 void tc_tail_destroy(TcTailState* s);
 int tc_tail_num_partials(const TcTailState* s);
-// loss_partials: per-CTA unscaled loss partials [tc_tail_num_partials] or NULL.
+// loss_partials: workspace of 1024 floats (per-CTA unscaled partials + the arrival ticket, zeroed at create) or NULL;
+// loss: device scalar that the last CTA of the forward kernel writes (s * sum of the partials; no second launch).
 // z_mode = 1: logits-only forward, the dY buffer receives the logits (same layout and dtype); no targets, no loss.
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
-                    const float* bias, const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY,
+                    const float* bias, const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY,
                     float* logits_out, int z_mode, cudaStream_t st, int* n_launches);
 int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
                float* dbias, cudaStream_t st, int* n_launches);
@@ -37,7 +38,7 @@ int tc_head_create(TcHeadState** out, int d, int64_t L_h, int B_max, int device)
 void tc_head_destroy(TcHeadState* s);
 int tc_head_num_partials(const TcHeadState* s);
 int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const float* bias,
-                    const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
+                    const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY, float* logits_out,
                     cudaStream_t st, int* n_launches);
 int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const void* dY, void* dWh,
                      float* dbias, float* dX, int accumulate_dX, int deterministic, cudaStream_t st, int* n_launches);

@@ -68,7 +68,8 @@ struct FwdParams {
   const float* bias;       // [L] or null
   const int32_t* rowptr;   // [B+1] or null
   const int32_t* col;      // [nnz]
-  float* partials;         // [gridDim.x] unscaled loss partials, or null
+  float* partials;         // [1024] unscaled loss partials + ticket (finalize_loss_last_cta), or null
+  float* loss;             // device scalar: s * sum of the partials, written by the last CTA
   float* logits;           // [B][L] fp32 or null
   int write_dy;
   int z_mode;              // 1: the dY buffer receives the logits themselves (bf16, same layout); no targets, no loss
@@ -364,11 +365,13 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   tc_fence_before();
   __syncthreads();
   if (warp == EW + 4) { tc_fence_after(); tmem_dealloc<512>(tmem_base); }
-  if (threadIdx.x == 0 && p.partials) {
+  if (p.partials) {
     float t = 0.f;
+    if (threadIdx.x == 0) {
 #pragma unroll
-    for (int i = 0; i < EW; ++i) t += loss_red[i];
-    p.partials[blockIdx.x] = t;
+      for (int i = 0; i < EW; ++i) t += loss_red[i];
+    }
+    finalize_loss_last_cta(p.partials, t, p.s, p.loss);
   }
 }
 
@@ -401,7 +404,7 @@ int tc_tail_num_partials(const TcTailState* s) { return s->n_partials; }
 
 template <int G, int K>
 static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
-                      const int32_t* rowptr, const int32_t* col, float* partials, void* dY, float* logits, int z_mode, cudaStream_t st) {
+                      const int32_t* rowptr, const int32_t* col, float* partials, float* loss, void* dY, float* logits, int z_mode, cudaStream_t st) {
   using C = FwdCfg<G, K>;
   static_assert(C::SMEM <= 232448, "shared memory budget");
   CUtensorMap tmW, tmY;
@@ -422,7 +425,7 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
     tmY = tmW;
   }
   FwdParams p;
-  p.Xt = (const bf16*)Xt; p.idx = idx; p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = partials; p.logits = logits;
+  p.Xt = (const bf16*)Xt; p.idx = idx; p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = partials; p.loss = loss; p.logits = logits;
   p.write_dy = dY ? 1 : 0;
   p.z_mode = z_mode;
   p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NP = (p.NT + 1) / 2;
@@ -430,8 +433,6 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   p.L = sh.L; p.NG = sh.NG; p.label_offset = sh.label_offset; p.s = sh.s;
   if (p.NP > s->num_sms) { set_error("batch too large for the tcgen05 forward"); return HASTE_ERR_UNSUPPORTED; }
   const int grid = p.NP * p.S;
-  if (partials && grid < s->n_partials)   // partials beyond the grid stay zero from create / earlier calls: clear them
-    HASTE_CUDA_TRY(cudaMemsetAsync(partials + grid, 0, (size_t)(s->n_partials - grid) * sizeof(float), st));
   HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
   tc_fwd_kernel<G, K><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
   HASTE_LAUNCH_CHECK();
@@ -439,11 +440,11 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
 }
 
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
-                    const int32_t* rowptr, const int32_t* col, float* loss_partials, void* dY, float* logits_out,
+                    const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY, float* logits_out,
                     int z_mode, cudaStream_t st, int* n_launches) {
   *n_launches = 1;
 #define HASTE_FWD(G_, K_) \
-  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, dY, logits_out, z_mode, st)
+  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, loss, dY, logits_out, z_mode, st)
   HASTE_FWD(64, 128); HASTE_FWD(64, 64); HASTE_FWD(32, 64); HASTE_FWD(32, 128); HASTE_FWD(128, 64); HASTE_FWD(128, 128);
 #undef HASTE_FWD
   set_error("tcgen05 forward: unsupported (G, K)");

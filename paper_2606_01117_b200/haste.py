@@ -15,7 +15,7 @@ _DIR = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_DIR, "libhaste.so")
 
 HASTE_F32, HASTE_BF16 = 0, 1
-HASTE_IDX_SORTED_DISTINCT, HASTE_DETERMINISTIC, HASTE_FORCE_SIMT = 1, 2, 4
+HASTE_IDX_SORTED_DISTINCT, HASTE_DETERMINISTIC, HASTE_FORCE_SIMT, HASTE_XT_FROM_FORWARD = 1, 2, 4, 8
 HASTE_OK, HASTE_ERR_INVALID_ARG, HASTE_ERR_BAD_INDEX, HASTE_ERR_UNSUPPORTED, HASTE_ERR_CUDA, HASTE_ERR_NOMEM = 0, -1, -2, -3, -4, -5
 
 # Every symbol include/haste.h declares (tests check the library exports all of them).

@@ -297,3 +297,29 @@ def test_forward_logits_only(oracle, H, shape, with_bias):
     NG = -(-L // G)
     if NG * G > L:
         assert torch.count_nonzero(Z.view(NG, B, G)[NG - 1, :, L - (NG - 1) * G:]).item() == 0
+
+
+def test_xt_from_forward_flag(oracle, H):
+    """HASTE_XT_FROM_FORWARD: the backward reuses the forward's transposed copy of X (same handle, same X and B); results
+    are those of the default path, bit for bit (dW, db) -- and the default path does not depend on an earlier forward."""
+    from gpu_util import TailRun
+    B, d, L, G, K = 200, 256, 64 * 7 + 9, 64, 64
+    inp = synth.small_case(83, B, d, L, G, K, dtype="bf16", w_std=0.05)
+    a = TailRun(inp, G, flags=H.HASTE_XT_FROM_FORWARD, dw_dtype="f32")
+    fa = a.forward()
+    ba = a.backward()
+    b = TailRun(inp, G, dw_dtype="f32")
+    fb = b.forward()
+    bb = b.backward()
+    assert np.array_equal(fa["dY"], fb["dY"])
+    assert np.array_equal(ba["dW"], bb["dW"]) and np.array_equal(ba["db"], bb["db"])
+    assert a.bwd_launches == b.bwd_launches - 1
+    ref = oracle.tail_forward(inp.X, inp.idx, inp.W, inp.bias, inp.rowptr, inp.col, G)
+    bref = oracle.tail_backward(inp.X, inp.idx, inp.W, ref["dY"], G)
+    _check_backward(oracle, ba, bref, 5e-3, G)
+    # default path: a backward after a forward with ANOTHER X on the same handle still uses its own X
+    inp2 = synth.small_case(84, B, d, L, G, K, dtype="bf16", w_std=0.05)
+    from gpu_util import to_dev
+    b.layer.forward_loss(B, to_dev(inp2, "X"), b.idx, b.W, b.bias, b.rowptr, b.col, loss=None, dY=b.layer.alloc_dy(B))
+    bb2 = b.backward()
+    assert np.array_equal(bb2["dW"], bb["dW"])
