@@ -125,6 +125,17 @@ int haste_forward_loss(haste_layer_t* h, int B,
 int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W,
                          const float* bias /* [L] fp32 or NULL */, void* Z, void* stream);
 
+/* Fused top-k inference (Eq. 4: P@k needs only the k highest-scoring labels of a row): the forward
+ * contraction with an epilogue that keeps, per batch row, the k largest logits z[i,l] = bias[l] + <w_l, x_I> and their
+ * labels; the B x L logits are never written.  1 <= k <= 8.
+ *   out_val [B,k] fp32: the logits (fp32 accumulation of the bf16 products, not rounded), descending;
+ *   out_idx [B,k] int64: GLOBAL label ids (label_offset + l); ties go to the smaller label; -1 (value -inf) where the
+ *                        layer has fewer than k labels.
+ * tcgen05 kernel family only (HASTE_ERR_UNSUPPORTED otherwise).  The first call allocates a workspace of
+ * num_SMs * 32 KiB in the handle. */
+int haste_forward_topk(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W,
+                       const float* bias /* [L] fp32 or NULL */, int k, float* out_val, int64_t* out_idx, void* stream);
+
 /* Backward from a dY in the library layout. */
 int haste_backward(haste_layer_t* h, int B,
                    const void* X, const int32_t* idx, const void* W, const void* dY,

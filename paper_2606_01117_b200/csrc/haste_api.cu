@@ -92,6 +92,8 @@ struct haste_layer {
   float* partials;  // [n_partials] per-CTA loss partials (tcgen05 family)
   int n_partials;
   int* flag;        // validate_index result
+  float* topk_val;  // fused top-k candidates [num_SMs][4 sets][128][8] (allocated on first use)
+  int* topk_idx;
   TcTailState* tc;  // tcgen05 family state (tensor maps, counters) or NULL
   int last_launches;
   Profiler* prof;
@@ -216,7 +218,7 @@ int haste_destroy(haste_layer_t* h) {
   DeviceGuard guard(h->device);
   if (h->tc) tc_tail_destroy(h->tc);
   if (h->prof) { h->prof->destroy(); delete h->prof; }
-  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->dx_part); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag);
+  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->dx_part); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag); cudaFree(h->topk_val); cudaFree(h->topk_idx);
   delete h;
   return HASTE_OK;
 }
@@ -291,7 +293,7 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
     int n = 0;
     pf.begin(HASTE_KERNEL_FORWARD, st);
     rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, loss, dY,
-                         logits_out, 0, st, &n);       // the kernel's last CTA writes the loss
+                         logits_out, 0, nullptr, nullptr, nullptr, st, &n);       // the kernel's last CTA writes the loss
     if (rc) return rc;
     pf.end(HASTE_KERNEL_FORWARD, st);
     h->last_launches += n;
@@ -338,10 +340,55 @@ int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* 
   pf.end(HASTE_KERNEL_PREP_FWD, st);
   int n = 0;
   pf.begin(HASTE_KERNEL_FORWARD, st);
-  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, nullptr, Z, nullptr, 1, st, &n);
+  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, nullptr, Z, nullptr, 1, nullptr, nullptr, nullptr, st, &n);
   if (rc) return rc;
   pf.end(HASTE_KERNEL_FORWARD, st);
   h->last_launches += n;
+  return HASTE_OK;
+}
+
+int haste_forward_topk(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias, int k,
+                       float* out_val, int64_t* out_idx, void* stream) {
+  int rc = check_call(h, B, "haste_forward_topk");
+  if (rc) return rc;
+  if (!X || !idx || !W || !out_val || !out_idx) { set_error("haste_forward_topk: X, idx, W, out_val and out_idx are required"); return HASTE_ERR_INVALID_ARG; }
+  if (k < 1 || k > 8) { set_error("haste_forward_topk: k must be in [1, 8]"); return HASTE_ERR_INVALID_ARG; }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(idx)) { set_error("haste_forward_topk: X, W and idx must be 16-byte aligned"); return HASTE_ERR_INVALID_ARG; }
+  if (h->family != 1) { set_error("haste_forward_topk: only the tcgen05 kernel family has the fused top-k forward"); return HASTE_ERR_UNSUPPORTED; }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const TailShape sh = make_shape(h, B);
+  Profiler& pf = *h->prof;
+  h->last_launches = 0;
+  if (B == 0) return HASTE_OK;
+  if (!h->topk_val) {
+    const size_t n = (size_t)tc_tail_num_sms(h->tc) * 4 * 128 * 8;
+    if (cudaMalloc(&h->topk_val, n * 4) != cudaSuccess || cudaMalloc(&h->topk_idx, n * 4) != cudaSuccess) {
+      set_error("haste_forward_topk: workspace allocation failed");
+      return HASTE_ERR_NOMEM;
+    }
+  }
+  if (h->NG == 0) {     // no labels: every slot empty
+    HASTE_CUDA_TRY(cudaMemsetAsync(out_idx, 0xff, (size_t)B * k * 8, st));
+    HASTE_CUDA_TRY(cudaMemsetAsync(out_val, 0xff, (size_t)B * k * 4, st));
+    return HASTE_OK;
+  }
+  pf.begin(HASTE_KERNEL_PREP_FWD, st);
+  rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+  if (rc) return rc;
+  pf.end(HASTE_KERNEL_PREP_FWD, st);
+  int n = 0;
+  TopkGeom geom;
+  geom.k = k;
+  pf.begin(HASTE_KERNEL_FORWARD, st);
+  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 2, h->topk_val, h->topk_idx,
+                       &geom, st, &n);
+  if (rc) return rc;
+  rc = launch_topk_merge(h->topk_val, h->topk_idx, geom.NP, geom.S, geom.NSET, ceil_div(B, 128), B, k, h->cfg.label_offset, out_val,
+                         out_idx, st);
+  if (rc) return rc;
+  pf.end(HASTE_KERNEL_FORWARD, st);
+  h->last_launches = n + 2;
   return HASTE_OK;
 }
 

@@ -10,6 +10,9 @@ namespace haste {
 int launch_transpose_pad(haste_dtype_t dt, const void* X, void* Xt, int B, int d, int Bpad, int Bzero, cudaStream_t st);
 // dX[b][f] (=|+=) dXt[f][b]
 int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st);
+// fused top-k: merge the forward kernel's per-thread candidates into the k best (value, global label id) per batch row
+int launch_topk_merge(const float* cand_val, const int* cand_idx, int NP, int S, int NSET, int NT, int B, int k,
+                      int64_t label_offset, float* out_val, int64_t* out_idx, cudaStream_t st);
 int launch_reduce_dx_parts(const float* part, float* dXt, int d, int Bpad, int NT, int S, cudaStream_t st);
 int launch_finalize_loss(const double* acc, const float* partials, int n_partials, float scale, float* loss, cudaStream_t st);
 int launch_dy_unpack(haste_dtype_t dt, const void* dY, float* out_BL, int B, int64_t L, int G, cudaStream_t st);

@@ -14,12 +14,15 @@ bool tc_tail_supported(const haste_config_t& cfg, int device);
 int tc_tail_create(TcTailState** out, const haste_config_t& cfg, int Bpad, int device);
 void tc_tail_destroy(TcTailState* s);
 int tc_tail_num_partials(const TcTailState* s);
+// geometry of the forward launch, for the merge of the fused top-k candidates (launch_topk_merge)
+struct TopkGeom { int k; int NP, S, NSET; };     // k: in (the caller's k, picks the list length); the rest: out
 // loss_partials: workspace of 1024 floats (per-CTA unscaled partials + the arrival ticket, zeroed at create) or NULL;
 // loss: device scalar that the last CTA of the forward kernel writes (s * sum of the partials; no second launch).
 // z_mode = 1: logits-only forward, the dY buffer receives the logits (same layout and dtype); no targets, no loss.
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
                     const float* bias, const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY,
-                    float* logits_out, int z_mode, cudaStream_t st, int* n_launches);
+                    float* logits_out, int z_mode, float* topk_val, int* topk_idx, TopkGeom* geom, cudaStream_t st, int* n_launches);
+// z_mode = 2: fused top-k; topk_val / topk_idx: [grid][sets][128][8] candidate workspace (grid <= num SMs, sets <= 4)
 int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
                float* dbias, cudaStream_t st, int* n_launches);
 // dx_part: null, or (HASTE_DETERMINISTIC) private partial tiles [tc_tail_dx_parts()][d][128] fp32, zeroed by the caller: the kernel

@@ -20,6 +20,7 @@
 #include "tc_common.cuh"
 #include "tc_epilogue.cuh"
 #include "tc_kernels.h"
+#include <cmath>
 
 namespace haste {
 
@@ -73,6 +74,9 @@ struct FwdParams {
   float* logits;           // [B][L] fp32 or null
   int write_dy;
   int z_mode;              // 1: the dY buffer receives the logits themselves (bf16, same layout); no targets, no loss
+                           // 2: nothing is written but the per-thread top-8 logits of each batch row (topk_val / topk_idx)
+  float* topk_val;         // [gridDim.x][epilogue sets][128 rows][8] candidate logits (fp32), descending; -inf = none
+  int* topk_idx;           // same shape: label index inside this layer
   int B, Bpad, NT, NP, S;  // NT batch tiles of 128; NP tile pairs; S group stripes (grid = NP*S)
   int64_t L, NG, label_offset;
   float s;
@@ -98,7 +102,9 @@ template <int G, int K> struct FwdCfg {
   static constexpr int THREADS = (4 * NSET + 6) * 32;
 };
 
-template <int G, int K>
+// TOPK > 0: the fused top-k instances (z_mode 2; candidate lists of TOPK = 5 or 8 entries per thread) are kernels of their
+// own, so that the lists cost the training kernel (TOPK = 0) no registers
+template <int G, int K, int TOPK>
 __global__ void __launch_bounds__(FwdCfg<G, K>::THREADS, 1)
 tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmY, const FwdParams p) {
   using C = FwdCfg<G, K>;
@@ -246,6 +252,12 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     }
     float loss_local = 0.f;
     const float hs = 0.5f * p.s;
+    // z_mode 2 (fused top-k): the 8 largest logits this thread has seen for its batch row, descending
+    constexpr int KL = TOPK > 0 ? TOPK : 1;
+    float tv[KL];
+    int ti[KL];
+#pragma unroll
+    for (int i = 0; i < KL; ++i) { tv[i] = -INFINITY; ti[i] = -1; }
     // this warp's 32 rows of the half's staging tile(s); rows are 128 B (G >= 64) or 64 B (G = 32)
     constexpr int ROWB = G >= 64 ? 128 : 64;
     const uint32_t stage_w = sbase + C::OFF_ST + set * C::ST_BYTES + q * 32 * ROWB;
@@ -309,7 +321,41 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         float* zout = (p.logits && valid_row) ? p.logits + (size_t)b * p.L + g * G + sc * 32 : nullptr;
         const int nvalid = nl - sc * 32;
         const uint32_t sb = sbias_w + sc * 128;
-        if (p.z_mode) {           // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
+        if constexpr (TOPK > 0) { // fused top-k: nothing leaves the chip but the row's candidates
+          // A thread inserts ~KL ln(n / KL) times over the n labels it sees, so most runs of 8 logits hold nothing above its
+          // KL-th best: four 3-input maxima per run find that out, and only the runs that do are looked at one by one.
+#pragma unroll
+          for (int r8 = 0; r8 < 4; ++r8) {
+            float z[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const int jj = r8 * 8 + j;
+              z[j] = __uint_as_float(v[jj]);
+              if (p.bias) {
+                float b0;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(b0) : "r"(sb + jj * 4));
+                z[j] += b0;
+              }
+              if (jj >= nvalid) z[j] = -INFINITY;
+            }
+            const float m = max3(max3(z[0], z[1], z[2]), max3(z[3], z[4], z[5]), fmaxf(z[6], z[7]));
+            if (m > tv[KL - 1]) {
+              const int l0 = (int)(g * G) + sc * 32 + r8 * 8;
+#pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                if (z[j] > tv[KL - 1]) {             // insert into the descending list (stable: earlier labels win ties)
+                  tv[KL - 1] = z[j]; ti[KL - 1] = l0 + j;
+#pragma unroll
+                  for (int i = KL - 1; i > 0; --i)
+                    if (tv[i] > tv[i - 1]) {
+                      const float a = tv[i]; tv[i] = tv[i - 1]; tv[i - 1] = a;
+                      const int b_ = ti[i]; ti[i] = ti[i - 1]; ti[i - 1] = b_;
+                    }
+                }
+              }
+            }
+          }
+        } else if (p.z_mode) {    // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
 #pragma unroll
           for (int j = 0; j < 32; j += 2) {
             float z0 = __uint_as_float(v[j]), z1 = __uint_as_float(v[j + 1]);
@@ -356,6 +402,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
     }
     if (lane == 0) bulk_wait<0>();
+    if constexpr (TOPK > 0) {
+      const size_t o = (((size_t)blockIdx.x * C::NSET + set) * 128 + row) * 8;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { p.topk_val[o + i] = (valid_row && i < KL) ? tv[i < KL ? i : 0] : -INFINITY; p.topk_idx[o + i] = i < KL ? ti[i < KL ? i : 0] : -1; }
+    }
     if (!valid_row) loss_local = 0.f;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) loss_local += __shfl_xor_sync(0xffffffffu, loss_local, o);
@@ -404,7 +455,8 @@ int tc_tail_num_partials(const TcTailState* s) { return s->n_partials; }
 
 template <int G, int K>
 static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
-                      const int32_t* rowptr, const int32_t* col, float* partials, float* loss, void* dY, float* logits, int z_mode, cudaStream_t st) {
+                      const int32_t* rowptr, const int32_t* col, float* partials, float* loss, void* dY, float* logits, int z_mode,
+                      float* topk_val, int* topk_idx, TopkGeom* geom, cudaStream_t st) {
   using C = FwdCfg<G, K>;
   static_assert(C::SMEM <= 232448, "shared memory budget");
   CUtensorMap tmW, tmY;
@@ -427,24 +479,34 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   FwdParams p;
   p.Xt = (const bf16*)Xt; p.idx = idx; p.bias = bias; p.rowptr = rowptr; p.col = col; p.partials = partials; p.loss = loss; p.logits = logits;
   p.write_dy = dY ? 1 : 0;
-  p.z_mode = z_mode;
+  p.z_mode = z_mode; p.topk_val = topk_val; p.topk_idx = topk_idx;
   p.B = sh.B; p.Bpad = sh.Bpad; p.NT = ceil_div(sh.B, 128); p.NP = (p.NT + 1) / 2;
   p.S = (int)std::min<int64_t>(sh.NG, std::max(1, s->num_sms / p.NP));
   p.L = sh.L; p.NG = sh.NG; p.label_offset = sh.label_offset; p.s = sh.s;
   if (p.NP > s->num_sms) { set_error("batch too large for the tcgen05 forward"); return HASTE_ERR_UNSUPPORTED; }
   const int grid = p.NP * p.S;
-  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-  tc_fwd_kernel<G, K><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+  const int topk_k = geom ? geom->k : 0;
+  if (geom) { geom->NP = p.NP; geom->S = p.S; geom->NSET = C::NSET; }
+  if (z_mode == 2 && topk_k <= 5) {
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+    tc_fwd_kernel<G, K, 5><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+  } else if (z_mode == 2) {
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+    tc_fwd_kernel<G, K, 8><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+  } else {
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+    tc_fwd_kernel<G, K, 0><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+  }
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }
 
 int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
                     const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY, float* logits_out,
-                    int z_mode, cudaStream_t st, int* n_launches) {
+                    int z_mode, float* topk_val, int* topk_idx, TopkGeom* geom, cudaStream_t st, int* n_launches) {
   *n_launches = 1;
 #define HASTE_FWD(G_, K_) \
-  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, loss, dY, logits_out, z_mode, st)
+  if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, loss, dY, logits_out, z_mode, topk_val, topk_idx, geom, st)
   HASTE_FWD(64, 128); HASTE_FWD(64, 64); HASTE_FWD(32, 64); HASTE_FWD(32, 128); HASTE_FWD(128, 64); HASTE_FWD(128, 128);
 #undef HASTE_FWD
   set_error("tcgen05 forward: unsupported (G, K)");

@@ -3,6 +3,7 @@
 //   contiguous rows (gather-once); dX^T -> dX; loss finalisation; dY
 //   layout pack/unpack; index validation.
 #include "kernels.h"
+#include <cmath>
 
 namespace haste {
 
@@ -100,6 +101,68 @@ __global__ void finalize_loss_kernel(const double* acc, const float* partials, i
 int launch_finalize_loss(const double* acc, const float* partials, int n_partials, float scale, float* loss,
                          cudaStream_t st) {
   finalize_loss_kernel<<<1, 256, 0, st>>>(acc, partials, n_partials, scale, loss);
+  HASTE_LAUNCH_CHECK();
+  return HASTE_OK;
+}
+
+// ---------------------------------------------------------------------------------
+// Fused top-k inference (Eq. 4): merge of the candidates the forward kernel's epilogue threads kept
+// (8 per thread; tc_tail.cu, z_mode 2).  Batch row b sits in batch tile bt = b / 128 of tile pair pr = bt / 2; its
+// candidates are those of CTAs (stripe s, pair pr), s < S, and of the epilogue sets that worked on that tile (all sets if
+// the pair has one tile, the sets of matching parity if it has two).  One warp per row: every lane keeps the best 8 of
+// its share, then k rounds of a warp-wide arg-max (ties: larger value first, then smaller label index) pop the winners.
+// ---------------------------------------------------------------------------------
+__global__ void topk_merge_kernel(const float* __restrict__ cv, const int* __restrict__ ci, int NP, int S, int NSET, int NT,
+                                  int B, int k, int64_t label_offset, float* __restrict__ out_val, int64_t* __restrict__ out_idx) {
+  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (b >= B) return;
+  const int bt = b >> 7, r = b & 127, pr = bt >> 1;
+  const int ntp = min(2, NT - 2 * pr);
+  const int nsets = ntp == 2 ? NSET / 2 : NSET;           // sets that saw this tile
+  const int per_cta = nsets * 8, total = S * per_cta;
+  float tv[8];
+  int ti[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { tv[i] = -INFINITY; ti[i] = 0x7fffffff; }
+  for (int e = lane; e < total; e += 32) {
+    const int s = e / per_cta, w = e - s * per_cta;
+    const int set = ntp == 2 ? 2 * (w >> 3) + (bt & 1) : (w >> 3);
+    const size_t o = ((((size_t)s * NP + pr) * NSET + set) * 128 + r) * 8 + (w & 7);
+    const float z = cv[o];
+    const int l = ci[o];
+    if (l >= 0 && (z > tv[7] || (z == tv[7] && l < ti[7]))) {
+      tv[7] = z; ti[7] = l;
+#pragma unroll
+      for (int i = 7; i > 0; --i)
+        if (tv[i] > tv[i - 1] || (tv[i] == tv[i - 1] && ti[i] < ti[i - 1])) {
+          const float a = tv[i]; tv[i] = tv[i - 1]; tv[i - 1] = a;
+          const int c = ti[i]; ti[i] = ti[i - 1]; ti[i - 1] = c;
+        }
+    }
+  }
+  for (int round = 0; round < k; ++round) {
+    float bv = tv[0];
+    int bi = ti[0], bl = lane;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, o), ol = __shfl_xor_sync(0xffffffffu, bl, o);
+      if (ov > bv || (ov == bv && (oi < bi || (oi == bi && ol < bl)))) { bv = ov; bi = oi; bl = ol; }
+    }
+    if (lane == 0) {
+      out_val[(size_t)b * k + round] = bv;
+      out_idx[(size_t)b * k + round] = bi == 0x7fffffff ? -1 : label_offset + bi;
+    }
+    if (lane == bl) {       // the winner pops its head
+#pragma unroll
+      for (int i = 0; i < 7; ++i) { tv[i] = tv[i + 1]; ti[i] = ti[i + 1]; }
+      tv[7] = -INFINITY; ti[7] = 0x7fffffff;
+    }
+  }
+}
+int launch_topk_merge(const float* cv, const int* ci, int NP, int S, int NSET, int NT, int B, int k, int64_t label_offset,
+                      float* out_val, int64_t* out_idx, cudaStream_t st) {
+  topk_merge_kernel<<<ceil_div(B, 4), 128, 0, st>>>(cv, ci, NP, S, NSET, NT, B, k, label_offset, out_val, out_idx);
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }
