@@ -354,6 +354,28 @@ int haste_oracle_tail_batch_rows(int B, int d, int64_t L, int G, int K,
   return 0;
 }
 
+// ---------------------------------------------------------------------------
+// Optimizer step of the output layer: "SGD with momentum for the final layer".
+// The paper names the method and nothing else (no dampening, Nesterov or weight-decay statement), so this is the
+// textbook heavy-ball form, reading R13:
+//     g' = g + wd * w          (L2 weight decay, wd = 0 turns it off)
+//     v  <- mu * v + g'        (momentum buffer, starts at 0)
+//     w  <- w - lr * v
+// applied element by element to n parameters, everything in fp64.  Pins (tests/test_oracle_pins.py): mu = 0 is plain
+// gradient descent; two and n steps on a constant gradient have closed forms (w_n = w_0 - lr g sum_{t<n} (1-mu^{t+1})/(1-mu));
+// g = 0, mu = 0 shrinks w by (1 - lr wd).
+// ---------------------------------------------------------------------------
+int haste_oracle_sgd_momentum(int64_t n, const double* w, const double* g, const double* v, double lr, double mu, double wd,
+                              double* w_out, double* v_out) {
+  for (int64_t e = 0; e < n; ++e) {
+    const double gp = g[e] + wd * w[e];
+    const double vn = mu * v[e] + gp;
+    v_out[e] = vn;
+    w_out[e] = w[e] - lr * vn;
+  }
+  return 0;
+}
+
 // Scalar helpers exported so pins can check them against closed forms directly.
 double haste_oracle_softplus(double z) { return softplus(z); }
 double haste_oracle_sigmoid(double z) { return sigmoid(z); }

@@ -13,7 +13,7 @@ from . import build as _build
 
 __all__ = [
     "tail_forward", "tail_backward", "bruteforce", "head_forward", "head_backward",
-    "tail_points", "tail_label_rows", "tail_batch_rows", "softplus", "sigmoid", "rel_l2",
+    "tail_points", "tail_label_rows", "tail_batch_rows", "sgd_momentum", "softplus", "sigmoid", "rel_l2",
 ]
 
 _lib = None
@@ -199,3 +199,16 @@ def tail_batch_rows(X, idx, W, bias, rowptr, col, G, rows, label_offset=0, s=Non
         _p(X), _p(idx), _p(W), _p(bias), _p(rowptr), _p(col), ctypes.c_int64(label_offset), ctypes.c_double(s),
         ctypes.c_int64(n), _p(rows), _p(lr), _p(dX)))
     return dict(loss_rows=lr, dX=dX)
+
+
+def sgd_momentum(w, g, v, lr, mu, wd=0.0):
+    """One SGD-with-momentum step (heavy-ball form, reading R13) on arrays of any shape, fp64:
+    v' = mu v + (g + wd w);  w' = w - lr v'.  Returns (w', v')."""
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert w.shape == g.shape == v.shape
+    w_out, v_out = np.empty_like(w), np.empty_like(v)
+    _chk(_L().haste_oracle_sgd_momentum(ctypes.c_int64(w.size), _p(w), _p(g), _p(v), ctypes.c_double(lr), ctypes.c_double(mu),
+                                        ctypes.c_double(wd), _p(w_out), _p(v_out)))
+    return w_out, v_out

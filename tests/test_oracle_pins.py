@@ -332,3 +332,32 @@ def test_p10_expected_softplus_scale(oracle):
     f = oracle.tail_forward(inp.X, inp.idx, inp.W, None, inp.rowptr, inp.col, cfg.G, want_z=True, want_dY=False)
     per_logit = (f["loss"] * cfg.B + f["z"][_dense_targets(cfg.B, cfg.L, inp.rowptr, inp.col) > 0].sum()) / (cfg.B * cfg.L)
     assert abs(per_logit - (math.log(2.0) + cfg.K * 0.02 ** 2 / 8)) < 2e-4
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# SGD with momentum on the output layer (heavy-ball form, reading R13)
+# ------------------------------------------------------------------------------------------------------------------
+def test_sgd_momentum_closed_forms(oracle):
+    rng = np.random.RandomState(11)
+    w0 = rng.standard_normal((7, 5))
+    g = rng.standard_normal((7, 5))
+    lr, mu = 0.1, 0.9
+    # mu = 0, wd = 0: plain gradient descent
+    w1, v1 = oracle.sgd_momentum(w0, g, np.zeros_like(w0), lr, 0.0)
+    assert np.allclose(w1, w0 - lr * g, rtol=0, atol=1e-15) and np.allclose(v1, g, rtol=0, atol=0)
+    # constant gradient, n steps from v = 0:  v_n = g (1 - mu^n) / (1 - mu),  w_n = w_0 - lr g sum_{t=1..n} (1 - mu^t) / (1 - mu)
+    w, v = w0.copy(), np.zeros_like(w0)
+    for n in range(1, 6):
+        w, v = oracle.sgd_momentum(w, g, v, lr, mu)
+        assert np.allclose(v, g * (1 - mu ** n) / (1 - mu), rtol=1e-13, atol=0)
+        assert np.allclose(w, w0 - lr * g * sum((1 - mu ** t) / (1 - mu) for t in range(1, n + 1)), rtol=1e-12, atol=1e-14)
+        if n == 2:
+            assert np.allclose(w, w0 - lr * g * (2 + mu), rtol=1e-13, atol=1e-15)      # the two-step form, by hand
+    # g = 0, mu = 0: weight decay alone shrinks w by (1 - lr wd)
+    w1, _ = oracle.sgd_momentum(w0, np.zeros_like(w0), np.zeros_like(w0), lr, 0.0, wd=0.05)
+    assert np.allclose(w1, w0 * (1 - lr * 0.05), rtol=1e-15, atol=0)
+    # a hand-computed scalar: w = 2, g = 0.5, v = 1, lr = 0.1, mu = 0.9, wd = 0.01 -> g' = 0.52, v' = 1.42, w' = 1.858
+    w1, v1 = oracle.sgd_momentum(np.array([2.0]), np.array([0.5]), np.array([1.0]), 0.1, 0.9, wd=0.01)
+    assert abs(v1[0] - 1.42) < 1e-15 and abs(w1[0] - 1.858) < 1e-15
+    # the sign of the step: a positive gradient lowers the weight
+    assert oracle.sgd_momentum(np.array([0.0]), np.array([1.0]), np.array([0.0]), 1.0, 0.5)[0][0] == -1.0
