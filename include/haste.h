@@ -145,6 +145,19 @@ int haste_backward(haste_layer_t* h, int B,
                    int accumulate_dX, /* 0: overwrite dX; 1: add to its contents                  */
                    void* stream);
 
+/* Backward with the optimizer step of the output layer fused into the weight-gradient kernel: "SGD with
+ * momentum for the final layer" (the heavy-ball form, optional L2 decay -- DESIGN.md reading R13):
+ *     g = dW[l,j] (never written to memory)      v[l,j] <- mu v[l,j] + g + weight_decay W[l,j]
+ *     W[l,j] <- W[l,j] - lr v[l,j]   (fp32 arithmetic, W rounded once to bf16)
+ * and for the bias, if given: vb[l] <- mu vb[l] + db[l];  b[l] <- b[l] - lr vb[l]  (no decay).
+ * dX, if wanted, is computed FIRST, from W as the forward used it.  W [L,K] bf16 and momentum [L,K] fp32 are read and
+ * written in place (16-byte aligned); bias / bias_momentum [L] fp32 both given or both NULL.  A call with B = 0 is a
+ * no-op.  tcgen05 kernel family without HASTE_DETERMINISTIC, (G, K) other than (32, 128): otherwise HASTE_ERR_UNSUPPORTED
+ * and nothing is modified. */
+int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* idx, void* W, const void* dY,
+                       float* momentum, float* bias, float* bias_momentum, float lr, float mu, float weight_decay,
+                       float* dX, int accumulate_dX, void* stream);
+
 /* dY layout helpers: library layout <-> plain [B,L] row-major fp32. */
 int haste_dy_unpack(const haste_layer_t* h, int B, const void* dY, float* out_BL, void* stream);
 int haste_dy_pack(const haste_layer_t* h, int B, const float* in_BL, void* dY, void* stream);

@@ -471,6 +471,57 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
   return HASTE_OK;
 }
 
+int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* idx, void* W, const void* dY, float* momentum,
+                       float* bias, float* bias_momentum, float lr, float mu, float weight_decay, float* dX, int accumulate_dX,
+                       void* stream) {
+  int rc = check_call(h, B, "haste_backward_sgd");
+  if (rc) return rc;
+  if (!X || !idx || !W || !dY || !momentum) { set_error("haste_backward_sgd: X, idx, W, dY and momentum are required"); return HASTE_ERR_INVALID_ARG; }
+  if ((bias == nullptr) != (bias_momentum == nullptr)) { set_error("haste_backward_sgd: bias and bias_momentum go together"); return HASTE_ERR_INVALID_ARG; }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(dY) || !aligned16(momentum) || !aligned16(idx)) {
+    set_error("haste_backward_sgd: X, W, idx, dY and momentum must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (h->family != 1 || h->dx_part) {
+    set_error("haste_backward_sgd: needs the tcgen05 kernel family (bf16, G in {32,64,128}, K in {64,128}) without HASTE_DETERMINISTIC");
+    return HASTE_ERR_UNSUPPORTED;
+  }
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const TailShape sh = make_shape(h, B);
+  Profiler& pf = *h->prof;
+  h->last_launches = 0;
+  if (B == 0 || h->NG == 0) return HASTE_OK;     // an empty batch has a zero gradient: with mu v the step would still move W; defined as a no-op
+  pf.begin(HASTE_KERNEL_PREP_BWD, st);
+  if (!(h->cfg.flags & HASTE_XT_FROM_FORWARD)) {
+    rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+    if (rc) return rc;
+    h->last_launches++;
+  }
+  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+  pf.end(HASTE_KERNEL_PREP_BWD, st);
+  int n = 0;
+  if (dX) {        // the input gradient first: it needs W as it was in the forward, the update below overwrites it
+    pf.begin(HASTE_KERNEL_DX, st);
+    rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, nullptr, st, &n);
+    if (rc) return rc;
+    h->last_launches += n;
+    pf.end(HASTE_KERNEL_DX, st);
+    pf.begin(HASTE_KERNEL_POST_BWD, st);
+    rc = launch_untranspose_f32(h->dXt, dX, B, sh.d, h->Bpad, accumulate_dX, st);
+    if (rc) return rc;
+    h->last_launches++;
+    pf.end(HASTE_KERNEL_POST_BWD, st);
+  }
+  pf.begin(HASTE_KERNEL_DW, st);
+  rc = tc_tail_dw_sgd(h->tc, sh, h->Xt, idx, dY, W, momentum, bias, bias_momentum, lr, mu, weight_decay, st, &n);
+  if (rc == HASTE_ERR_UNSUPPORTED) set_error("haste_backward_sgd: no fused kernel for G = %d, K = %d", sh.G, sh.K);
+  if (rc) return rc;
+  h->last_launches += n;
+  pf.end(HASTE_KERNEL_DW, st);
+  return HASTE_OK;
+}
+
 int haste_set_profiling(haste_layer_t* h, int depth) {
   if (!h) { set_error("haste_set_profiling: handle is NULL"); return HASTE_ERR_INVALID_ARG; }
   DeviceGuard guard(h->device);

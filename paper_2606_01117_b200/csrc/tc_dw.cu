@@ -15,6 +15,7 @@
 // rows; a thread owns one label, so a dW row is written as it is stored), warps 4-7 gather producers,
 // warp 8 MMA issuer, warp 9 TMA loader of dY.
 #include <algorithm>
+#include <cstring>
 
 #include "tc_common.cuh"
 #include "tc_kernels.h"
@@ -27,11 +28,17 @@ struct DwParams {
   const int32_t* idx;   // [NG][K]
   float* dbias;         // [L] or null
   int write_dw;
+  // SGD instance (haste_backward_sgd): the gradient never leaves the chip; W and the momentum are updated in place
+  bf16* W;              // [L][K] in/out
+  float* mom;           // [L][K] fp32 momentum buffer, in/out
+  float* bias;          // [L] in/out or null
+  float* bmom;          // [L] in/out or null (required with bias)
+  float lr, mu, wd;
   int B, Bpad, NKB;     // NKB = ceil(B / 128) k-blocks
   int64_t L, NG;
 };
 
-template <int G, int K, bool F32> struct DwCfg {
+template <int G, int K, bool F32, bool SGD = false> struct DwCfg {
   // G = 32: two consecutive groups form one virtual group of GV = 64 labels and KV = 2K slots (their idx rows are
   // adjacent in memory, so are their labels).  D [64 x 2K] then holds dW_g in rows 0-31 x columns [0,K) and dW_{g+1}
   // in rows 32-63 x columns [K,2K); the off-diagonal blocks are computed and ignored (the tensor pipe has the room).
@@ -74,10 +81,10 @@ __device__ __forceinline__ uint32_t tmem_ld1(uint32_t taddr) {
   return v;
 }
 
-template <int G, int K, bool F32>
+template <int G, int K, bool F32, bool SGD>
 __global__ void __launch_bounds__(320, 1)
 tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmO, const DwParams p) {
-  using C = DwCfg<G, K, F32>;
+  using C = DwCfg<G, K, F32, SGD>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const uint32_t sbase = smem_u32(smem);
@@ -228,7 +235,82 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * C::TS;
       const uint32_t tcol = taddr + (C::PAIR && q >= 2 ? K : 0);   // PAIR: quadrants 2, 3 hold group 2v+1, whose dW sits in columns [K, 2K)
-      if (p.write_dw) {
+      if constexpr (SGD) {
+        // v <- mu v + (g + wd w);  w <- w - lr v   (reading R13).  The accumulator rows ARE the
+        // gradient rows, so dW is never written: 32 columns at a time they go through the warp's staging rows (as for a
+        // dW store), and the warp then walks them in memory order -- 8 lanes per label row, 16 bytes of momentum and 8 of
+        // W each -- so that every global access is a run of whole 128-byte lines and all of a pass's loads are in flight
+        // together.  The next group's rows are pulled into L2 meanwhile.
+        const int64_t l0 = g * C::GV + q * C::RW;                    // first label row of this warp
+        const int64_t l = l0 + lane;
+        const bool own = lane < C::RW && l < p.L;
+        if (i + 1 < n_my) {
+          const int64_t ln0 = l0 + (int64_t)gridDim.x * C::GV;
+          constexpr int WL = K * 2 / 128, ML = K * 4 / 128;          // 128-byte lines per row of W / of the momentum
+          for (int e = lane; e < C::RW * (WL + ML); e += 32) {
+            const int r = e / (WL + ML), b = e - r * (WL + ML);
+            if (ln0 + r < p.L) {
+              const char* a = b < WL ? reinterpret_cast<const char*>(p.W + (ln0 + r) * K) + b * 128
+                                     : reinterpret_cast<const char*>(p.mom + (ln0 + r) * K) + (b - WL) * 128;
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+            }
+          }
+        }
+#pragma unroll 1
+        for (int c = 0; c < K / 32; ++c) {
+          uint32_t gq[32];
+          tmem_ld32(tcol + c * 32, gq);
+          tmem_ld_wait();
+          __syncwarp();                                              // the previous pass has read the staging rows
+#pragma unroll
+          for (int ch = 0; ch < 8; ++ch)
+            sts128(sbuf0 + lane * 128 + ((ch ^ swz) << 4), gq[4 * ch], gq[4 * ch + 1], gq[4 * ch + 2], gq[4 * ch + 3]);
+          __syncwarp();
+          constexpr int NIT = C::RW / 4;                             // (RW rows x 8 chunks of 4 columns) / 32 lanes
+#pragma unroll
+          for (int h0 = 0; h0 < NIT; h0 += 4) {
+            float4 g4[4], m4[4];
+            uint2 w2[4];
+            bool ok[4];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+              const int e = lane + 32 * (h0 + t), r = e >> 3, c16 = e & 7;
+              ok[t] = l0 + r < p.L;
+              g4[t] = lds128f(sbuf0 + r * 128 + ((c16 ^ (r & 7)) << 4));
+              if (ok[t]) {
+                const size_t o = (size_t)(l0 + r) * K + c * 32 + c16 * 4;
+                m4[t] = __ldcg(reinterpret_cast<const float4*>(p.mom + o));
+                w2[t] = __ldcg(reinterpret_cast<const uint2*>(p.W + o));
+              }
+            }
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+              if (!ok[t]) continue;
+              const int e = lane + 32 * (h0 + t), r = e >> 3, c16 = e & 7;
+              const size_t o = (size_t)(l0 + r) * K + c * 32 + c16 * 4;
+              const float w0 = __uint_as_float(w2[t].x << 16), w1 = __uint_as_float(w2[t].x & 0xffff0000u);
+              const float w2f = __uint_as_float(w2[t].y << 16), w3 = __uint_as_float(w2[t].y & 0xffff0000u);
+              float4 v;
+              v.x = fmaf(p.mu, m4[t].x, fmaf(p.wd, w0, g4[t].x));
+              v.y = fmaf(p.mu, m4[t].y, fmaf(p.wd, w1, g4[t].y));
+              v.z = fmaf(p.mu, m4[t].z, fmaf(p.wd, w2f, g4[t].z));
+              v.w = fmaf(p.mu, m4[t].w, fmaf(p.wd, w3, g4[t].w));
+              *reinterpret_cast<float4*>(p.mom + o) = v;
+              *reinterpret_cast<uint2*>(p.W + o) = make_uint2(dw_pack_bf16x2(fmaf(-p.lr, v.x, w0), fmaf(-p.lr, v.y, w1)),
+                                                              dw_pack_bf16x2(fmaf(-p.lr, v.z, w2f), fmaf(-p.lr, v.w, w3)));
+            }
+          }
+        }
+        if (p.bias) {       // bias: the same step without weight decay; db is accumulator column KV
+          const uint32_t v = tmem_ld1(taddr + C::KV);
+          tmem_ld_wait();
+          if (own) {
+            const float vb = fmaf(p.mu, p.bmom[l], __uint_as_float(v));
+            p.bmom[l] = vb;
+            p.bias[l] = fmaf(-p.lr, vb, p.bias[l]);
+          }
+        }
+      } else if (p.write_dw) {
 #pragma unroll 1
         for (int c = 0; c < C::NBOX; ++c, ++nstore) {
           uint32_t out[32];
@@ -260,7 +342,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           }
         }
       }
-      if (p.dbias) {
+      if (!SGD && p.dbias) {
         const uint32_t v = tmem_ld1(taddr + C::KV);
         tmem_ld_wait();
         const int64_t l = g * C::GV + q * C::RW + lane;
@@ -278,10 +360,12 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   if (warp == 8) { tc_fence_after(); tmem_dealloc<2 * C::TS>(tmem_base); }
 }
 
-template <int G, int K, bool F32>
+struct DwSgd { void* W; float* mom; float* bias; float* bmom; float lr, mu, wd; };
+
+template <int G, int K, bool F32, bool SGD = false>
 static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
-                     float* dbias, cudaStream_t st) {
-  using C = DwCfg<G, K, F32>;
+                     float* dbias, cudaStream_t st, const DwSgd* sgd = nullptr) {
+  using C = DwCfg<G, K, F32, SGD>;
   static_assert(C::SMEM <= 232448, "shared memory budget");
   CUtensorMap tmY, tmO;
   {
@@ -302,11 +386,13 @@ static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const 
     tmO = tmY;
   }
   DwParams p;
+  memset(&p, 0, sizeof(p));
   p.Xt = (const bf16*)Xt; p.idx = idx; p.dbias = dbias; p.write_dw = dW ? 1 : 0;
+  if (SGD) { p.W = (bf16*)sgd->W; p.mom = sgd->mom; p.bias = sgd->bias; p.bmom = sgd->bmom; p.lr = sgd->lr; p.mu = sgd->mu; p.wd = sgd->wd; }
   p.B = sh.B; p.Bpad = sh.Bpad; p.NKB = ceil_div(sh.B, 128); p.L = sh.L; p.NG = sh.NG;
   const int grid = (int)std::min<int64_t>(C::PAIR ? (sh.NG + 1) / 2 : sh.NG, s->num_sms);
-  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dw_kernel<G, K, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-  tc_dw_kernel<G, K, F32><<<grid, 320, C::SMEM, st>>>(tmY, tmO, p);
+  HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dw_kernel<G, K, F32, SGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+  tc_dw_kernel<G, K, F32, SGD><<<grid, 320, C::SMEM, st>>>(tmY, tmO, p);
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }
@@ -322,6 +408,19 @@ int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_
   HASTE_DW(64, 128); HASTE_DW(64, 64); HASTE_DW(128, 64); HASTE_DW(128, 128); HASTE_DW(32, 64);
 #undef HASTE_DW
   return HASTE_ERR_UNSUPPORTED;   // G = 32 with K = 128 (the paired MMA would need N = 264): the caller runs the CUDA-core kernel
+}
+
+// the same contraction with the SGD-momentum step of the output layer as its epilogue: W [L,K] (bf16) and
+// mom [L,K] (fp32) updated in place, bias / bmom [L] too if given; the gradient is never written
+int tc_tail_dw_sgd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* W, float* mom,
+                   float* bias, float* bmom, float lr, float mu, float wd, cudaStream_t st, int* n_launches) {
+  *n_launches = 1;
+  const DwSgd sgd = {W, mom, bias, bmom, lr, mu, wd};
+#define HASTE_DWS(G_, K_) \
+  if (sh.G == G_ && sh.K == K_) return launch_dw<G_, K_, true, true>(s, sh, Xt, idx, dY, nullptr, nullptr, st, &sgd)
+  HASTE_DWS(64, 128); HASTE_DWS(64, 64); HASTE_DWS(128, 64); HASTE_DWS(128, 128); HASTE_DWS(32, 64);
+#undef HASTE_DWS
+  return HASTE_ERR_UNSUPPORTED;
 }
 
 }  // namespace haste

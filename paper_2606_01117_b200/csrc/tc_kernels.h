@@ -25,6 +25,9 @@ int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const i
 // z_mode = 2: fused top-k; topk_val / topk_idx: [grid][sets][128][8] candidate workspace (grid <= num SMs, sets <= 4)
 int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
                float* dbias, cudaStream_t st, int* n_launches);
+// dW with the SGD-momentum step of the output layer as its epilogue (tc_dw.cu): W, mom (and bias, bmom) updated in place
+int tc_tail_dw_sgd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* W, float* mom,
+                   float* bias, float* bmom, float lr, float mu, float wd, cudaStream_t st, int* n_launches);
 // dx_part: null, or (HASTE_DETERMINISTIC) private partial tiles [tc_tail_dx_parts()][d][128] fp32, zeroed by the caller: the kernel
 // then uses no float atomics and the caller sums the tiles of a batch tile in stripe order (launch_reduce_dx_parts)
 int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
