@@ -57,11 +57,18 @@ __device__ __forceinline__ float rcp_approx(float x) {
 }
 
 // 8 logits (J0 .. J0+7) of one batch row.  SL: one of them may be a positive of the row or a padding label (>= L).
-// sigma(z) = 1/2 + 1/2 tanh.approx(z/2), one MUFU op per logit (the caller has checked that this is good enough, see epi32).
+// The fast evaluation (the caller has checked |z| <= 2.5, see epi32): t = tanh.approx(z/2), ONE MUFU op per logit, and then
+//   dY = s sigma(z) = s/2 + (s/2) t                                   (minus s at a positive)
+//   loss term of a negative: softplus(z)  = -ln sigma(-z) = -ln(1/2 - t/2)
+//   loss term of a positive: softplus(-z) = -ln sigma(z)  = -ln(1/2 + t/2)
+// so the term is the log of ONE factor per logit, multiplied into the running product P (no max(z,0), no |t|, no sum): 3.5
+// instructions per logit in packed f32x2 form.  With |z| <= 2.5 a factor is >= 0.076: 16 of them cannot underflow, and the
+// 2.4e-4 absolute error of tanh.approx is at most 0.3 % of it.
 template <bool SL, bool BIAS, int J0>
 __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s, uint64_t half2,
-                                     uint64_t hs2, uint64_t (&R2)[2], uint64_t (&P2)[2], uint32_t (&out)[16], float* zout) {
+                                     uint64_t hs2, uint64_t (&P2)[2], uint32_t (&out)[16], float* zout) {
   uint64_t bv2[2] = {0ull, 0ull};
+  const uint64_t nhalf2 = pk2(-0.5f, -0.5f);
 #pragma unroll
   for (int j = J0; j < J0 + 8; j += 2) {
     if (BIAS && (j & 3) == 0) {
@@ -70,25 +77,32 @@ __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, ui
     }
     uint64_t z2 = pk2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]));
     if (BIAS) z2 = add2(z2, bv2[(j >> 1) & 1]);
-    float z0, z1, d0, d1, f0, f1;
-    upk2(z2, z0, z1);
     float zh0, zh1;
     upk2(mul2(z2, half2), zh0, zh1);
-    const float t0 = tanh_approx(zh0), t1 = tanh_approx(zh1);
-    upk2(fma2(pk2(t0, t1), hs2, hs2), d0, d1);
-    f0 = fmaf(fabsf(t0), 0.5f, 0.5f); f1 = fmaf(fabsf(t1), 0.5f, 0.5f);
-    float r0 = fmaxf(z0, 0.f), r1 = fmaxf(z1, 0.f);
+    const uint64_t t2 = pk2(tanh_approx(zh0), tanh_approx(zh1));
+    uint64_t d2 = fma2(t2, hs2, hs2);              // s sigma(z)
+    uint64_t f2 = fma2(t2, nhalf2, half2);         // sigma(-z)
     if (SL) {
+      float d0, d1, f0, f1;
+      upk2(d2, d0, d1);
+      upk2(f2, f0, f1);
       const bool valid0 = j < nvalid, valid1 = j + 1 < nvalid;
-      if ((ymask >> j) & 1u) { d0 -= s; r0 -= z0; }
-      if ((ymask >> (j + 1)) & 1u) { d1 -= s; r1 -= z1; }
-      if (!valid0) { d0 = 0.f; f0 = 1.f; r0 = 0.f; }
-      if (!valid1) { d1 = 0.f; f1 = 1.f; r1 = 0.f; }
-      if (zout && valid0) zout[j] = z0;
-      if (zout && valid1) zout[j + 1] = z1;
+      if ((ymask >> j) & 1u) { d0 -= s; f0 = 1.f - f0; }
+      if ((ymask >> (j + 1)) & 1u) { d1 -= s; f1 = 1.f - f1; }
+      if (!valid0) { d0 = 0.f; f0 = 1.f; }
+      if (!valid1) { d1 = 0.f; f1 = 1.f; }
+      if (zout) {
+        float z0, z1;
+        upk2(z2, z0, z1);
+        if (valid0) zout[j] = z0;
+        if (valid1) zout[j + 1] = z1;
+      }
+      d2 = pk2(d0, d1);
+      f2 = pk2(f0, f1);
     }
-    P2[(j >> 1) & 1] = mul2(P2[(j >> 1) & 1], pk2(f0, f1));
-    R2[(j >> 1) & 1] = add2(R2[(j >> 1) & 1], pk2(r0, r1));
+    P2[(j >> 1) & 1] = mul2(P2[(j >> 1) & 1], f2);
+    float d0, d1;
+    upk2(d2, d0, d1);
     out[j >> 1] = pack_bf16x2(d0, d1);
   }
 }
@@ -129,8 +143,9 @@ static __device__ __noinline__ void epi32_wide(uint32_t* io, uint32_t sbias, int
 }
 
 // 32 logits of one batch row: z -> dY (bf16x2 packed) and the row's loss terms.
-//   softplus(z) = max(z,0) - ln( sigma(|z|) ), and the logs of a tile are taken once on the PRODUCT of the factors
-//   sigma(|z|) in [1/2,1]  (<= 16 per chain).
+//   Every loss term is minus the log of a factor in (0, 1], and the logs of a tile are taken once on the PRODUCT of the
+//   factors (<= 16 per chain P[k]); the wide evaluation also adds max(z,0) - y z into the sums R[k]:
+//   loss += (R[0]+R[1]+R[2]+R[3]) - ln 2 * log2(P[0] P[1] P[2] P[3]) at the caller.
 // sigma has two evaluations:
 //   fast: sigma(z) = 1/2 + 1/2 tanh.approx(z/2), ONE MUFU op per logit.  tanh.approx is good to 2^-11 RELATIVE to tanh,
 //         i.e. up to 2.4e-4 absolute on sigma: 0.3 % of sigma(-2.5) = 0.076, the size of the bf16 rounding of dY, and
@@ -142,14 +157,15 @@ static __device__ __noinline__ void epi32_wide(uint32_t* io, uint32_t sbias, int
 // SLOW: some label of this chunk may be a positive of some row of the warp, or the chunk holds padding labels (>= L), or
 // logits are wanted; the decision is then refined per 8 logits (warp-uniform), because the special-case code costs more
 // than the math itself and positives are rare (in the dense head ~70 % of the (warp, 128-label tile) pairs hold one).
-// Chains: logit jj feeds R[jj & 3] and P[jj & 3] (pair (j, j+1) = the two lanes of packed chain (j >> 1) & 1).
+// Chains: logit jj feeds P[jj & 3] (and, wide evaluation, R[jj & 3]); pair (j, j+1) = the two lanes of packed chain (j >> 1) & 1.
 template <bool SLOW, bool BIAS>
 __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
                                       float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
   // which evaluation: max |accumulator| over the warp's 32 x 32 logits (+ max |bias| of the 32 labels) against 2.5
-  float am = 0.f;
+  float a4[4] = {0.f, 0.f, 0.f, 0.f};          // four independent chains: one chain of 16 would be ~70 cycles of latency per chunk
 #pragma unroll
-  for (int j = 0; j < 32; j += 2) am = max3(am, fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1])));
+  for (int j = 0; j < 32; j += 2) a4[(j >> 1) & 3] = max3(a4[(j >> 1) & 3], fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1])));
+  float am = max3(fmaxf(a4[0], a4[1]), a4[2], a4[3]);
   if (BIAS) {
     float b;
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(b) : "r"(sbias + (threadIdx.x & 31) * 4));
@@ -168,19 +184,18 @@ __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, u
     for (int k = 0; k < 16; ++k) out[k] = io[40 + k];
     return;
   }
-  uint64_t R2[2] = {pk2(R[0], R[1]), pk2(R[2], R[3])}, P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};
+  uint64_t P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};      // (the fast path adds nothing to R: its loss terms are all in P)
   const uint64_t half2 = pk2(0.5f, 0.5f), hs2 = pk2(hs, hs);
 #define HASTE_EPI8(J0_)                                                                                             \
   if (SLOW) {                                                                                                        \
     const bool sl = __any_sync(0xffffffffu, ((ymask >> J0_) & 0xffu) != 0u) || nvalid < J0_ + 8 || zout != nullptr; \
-    if (sl) epi8<true, BIAS, J0_>(v, sbias, ymask, nvalid, s, half2, hs2, R2, P2, out, zout);                  \
-    else epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                        \
+    if (sl) epi8<true, BIAS, J0_>(v, sbias, ymask, nvalid, s, half2, hs2, P2, out, zout);                  \
+    else epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, P2, out, nullptr);                        \
   } else {                                                                                                           \
-    epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, R2, P2, out, nullptr);                             \
+    epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, P2, out, nullptr);                             \
   }
   HASTE_EPI8(0) HASTE_EPI8(8) HASTE_EPI8(16) HASTE_EPI8(24)
 #undef HASTE_EPI8
-  upk2(R2[0], R[0], R[1]); upk2(R2[1], R[2], R[3]);
   upk2(P2[0], P[0], P[1]); upk2(P2[1], P[2], P[3]);
 }
 

@@ -102,8 +102,8 @@ template <int G, int K> struct FwdCfg {
   static constexpr int THREADS = (4 * NSET + 6) * 32;
 };
 
-// TOPK > 0: the fused top-k instances (z_mode 2; candidate lists of TOPK = 5 or 8 entries per thread) are kernels of their
-// own, so that the lists cost the training kernel (TOPK = 0) no registers
+// TOPK > 0: the fused top-k instances (z_mode 2; candidate lists of TOPK = 5 or 8 entries per thread) and TOPK = -1: the
+// logits-only instance (z_mode 1) are kernels of their own, so that they cost the training kernel (TOPK = 0) no registers
 template <int G, int K, int TOPK>
 __global__ void __launch_bounds__(FwdCfg<G, K>::THREADS, 1)
 tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmY, const FwdParams p) {
@@ -355,7 +355,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
               }
             }
           }
-        } else if (p.z_mode) {    // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
+        } else if constexpr (TOPK < 0) {    // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
 #pragma unroll
           for (int j = 0; j < 32; j += 2) {
             float z0 = __uint_as_float(v[j]), z1 = __uint_as_float(v[j + 1]);
@@ -493,6 +493,9 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   } else if (z_mode == 2) {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
     tc_fwd_kernel<G, K, 8><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+  } else if (z_mode == 1) {
+    HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+    tc_fwd_kernel<G, K, -1><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
   } else {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
     tc_fwd_kernel<G, K, 0><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
