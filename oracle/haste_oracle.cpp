@@ -376,6 +376,99 @@ int haste_oracle_sgd_momentum(int64_t n, const double* w, const double* g, const
   return 0;
 }
 
+// ---------------------------------------------------------------------------
+// Group-shared rewiring, Algorithm 3, SURVEY.md 8(f3).  Step by step in the paper's order:
+//   1. scores   S[k,j] = mean over the labels l of group k of |w_l[j]|
+//   2. m = floor(NG * K * rho); mask M = the m smallest entries of S
+//   3. regrow   I_k[j] <- Unif{0..H-1} for every masked (k,j)
+//   4. reinit   w_l[j] <- 0  (zero mode)  or  Unif(-1/sqrt(F), 1/sqrt(F))  (random mode)
+// Readings (R15): a score decides an INTEGER (which slots are pruned), so it is computed the way the kernel
+// computes it -- fp32, labels added in ascending order, divided by the label count -- and ties are broken by the flat
+// index k*K + j (smaller first); the partial last group averages over the labels it has.  Random numbers come from a
+// counter-based generator both sides implement (SplitMix64 finaliser of seed + golden-ratio * (counter + 1)):
+//   regrown feature  u = floor(d * h / 2^64) = high 64 bits of h * d,      h = mix(seed, k*K + j)
+//   random weight    w = float(2 U - 1) * float(1/sqrt(K)) in fp32, U = (h >> 41) / 2^23,  h = mix(seed ^ 0x5851f42d4c957f2d, l*K + j)
+//                    (then rounded to bf16 by the caller when the layer stores bf16)
+// Optional extras, not in the paper (its Alg. 3 stops after step 4): momentum entries of reinitialised weights are set
+// to 0; `resort` != 0 re-sorts every touched idx row ascending (stable: ties keep their slot order) and permutes the W
+// (and momentum) columns of the group's labels with it -- the layer's function is invariant under slot permutations
+// (pin P8), and sorted rows are what the tcgen05 dX kernel's on-chip classes need.
+// ---------------------------------------------------------------------------
+static inline uint64_t rw_mix(uint64_t seed, uint64_t counter) {
+  uint64_t z = seed + 0x9e3779b97f4a7c15ULL * (counter + 1);
+  z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ULL;
+  z = (z ^ (z >> 27)) * 0x94d049bb133111ebULL;
+  return z ^ (z >> 31);
+}
+uint64_t haste_oracle_rewire_mix(uint64_t seed, uint64_t counter) { return rw_mix(seed, counter); }
+
+// scores_out [NG*K] fp32 (optional), mask_out [NG*K] bytes (optional).  W, mom are float32 arrays updated in place
+// (W holds the layer's values widened; the caller re-rounds random weights to the storage type).  Returns m, or -1.
+int64_t haste_oracle_rewire(int64_t L, int G, int K, int d, int32_t* idx, float* W, float* mom, double rho, int init_random,
+                            uint64_t seed, int resort, float* scores_out, unsigned char* mask_out) {
+  const int64_t NG = (L + G - 1) / G, n = NG * K;
+  std::vector<float> S((size_t)n);
+  for (int64_t k = 0; k < NG; ++k) {
+    const int64_t l0 = k * G, l1 = std::min<int64_t>(L, l0 + G);
+    for (int j = 0; j < K; ++j) {
+      float acc = 0.f;
+      for (int64_t l = l0; l < l1; ++l) acc = acc + std::fabs(W[l * K + j]);
+      S[(size_t)(k * K + j)] = acc / (float)(l1 - l0);
+    }
+  }
+  if (scores_out) std::copy(S.begin(), S.end(), scores_out);
+  const int64_t m = (int64_t)std::floor((double)n * rho);
+  std::vector<unsigned char> M((size_t)n, 0);
+  if (m > 0) {
+    std::vector<int64_t> order((size_t)n);
+    for (int64_t e = 0; e < n; ++e) order[(size_t)e] = e;
+    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return S[(size_t)a] < S[(size_t)b]; });
+    for (int64_t t = 0; t < m && t < n; ++t) M[(size_t)order[(size_t)t]] = 1;
+  }
+  if (mask_out) std::copy(M.begin(), M.end(), mask_out);
+  if (m <= 0) return 0;
+  const float r32 = (float)(1.0 / std::sqrt((double)K));
+  for (int64_t k = 0; k < NG; ++k) {
+    bool touched = false;
+    for (int j = 0; j < K; ++j) {
+      if (!M[(size_t)(k * K + j)]) continue;
+      touched = true;
+      const uint64_t h = rw_mix(seed, (uint64_t)(k * K + j));
+      idx[k * K + j] = (int32_t)(uint64_t)(((unsigned __int128)h * (unsigned __int128)(uint64_t)d) >> 64);
+      const int64_t l0 = k * G, l1 = std::min<int64_t>(L, l0 + G);
+      for (int64_t l = l0; l < l1; ++l) {
+        float w = 0.f;
+        if (init_random) {
+          const uint64_t hw = rw_mix(seed ^ 0x5851f42d4c957f2dULL, (uint64_t)(l * K + j));
+          const float a = (float)(2.0 * ((double)(hw >> 41) * (1.0 / 8388608.0)) - 1.0);
+          w = a * r32;
+        }
+        W[l * K + j] = w;
+        if (mom) mom[l * K + j] = 0.f;
+      }
+    }
+    if (touched && resort) {
+      std::vector<int> perm((size_t)K);
+      for (int j = 0; j < K; ++j) perm[(size_t)j] = j;
+      std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return idx[k * K + a] < idx[k * K + b]; });
+      std::vector<int32_t> irow((size_t)K);
+      for (int j = 0; j < K; ++j) irow[(size_t)j] = idx[k * K + perm[(size_t)j]];
+      for (int j = 0; j < K; ++j) idx[k * K + j] = irow[(size_t)j];
+      const int64_t l0 = k * G, l1 = std::min<int64_t>(L, l0 + G);
+      std::vector<float> row((size_t)K);
+      for (int64_t l = l0; l < l1; ++l) {
+        for (int j = 0; j < K; ++j) row[(size_t)j] = W[l * K + perm[(size_t)j]];
+        for (int j = 0; j < K; ++j) W[l * K + j] = row[(size_t)j];
+        if (mom) {
+          for (int j = 0; j < K; ++j) row[(size_t)j] = mom[l * K + perm[(size_t)j]];
+          for (int j = 0; j < K; ++j) mom[l * K + j] = row[(size_t)j];
+        }
+      }
+    }
+  }
+  return m;
+}
+
 // Scalar helpers exported so pins can check them against closed forms directly.
 double haste_oracle_softplus(double z) { return softplus(z); }
 double haste_oracle_sigmoid(double z) { return sigmoid(z); }

@@ -13,7 +13,7 @@ from . import build as _build
 
 __all__ = [
     "tail_forward", "tail_backward", "bruteforce", "head_forward", "head_backward",
-    "tail_points", "tail_label_rows", "tail_batch_rows", "sgd_momentum", "softplus", "sigmoid", "rel_l2",
+    "tail_points", "tail_label_rows", "tail_batch_rows", "sgd_momentum", "rewire", "rewire_mix", "softplus", "sigmoid", "rel_l2",
 ]
 
 _lib = None
@@ -212,3 +212,32 @@ def sgd_momentum(w, g, v, lr, mu, wd=0.0):
     _chk(_L().haste_oracle_sgd_momentum(ctypes.c_int64(w.size), _p(w), _p(g), _p(v), ctypes.c_double(lr), ctypes.c_double(mu),
                                         ctypes.c_double(wd), _p(w_out), _p(v_out)))
     return w_out, v_out
+
+
+def rewire_mix(seed, counter):
+    """The counter-based generator of the rewiring step (SplitMix64 finaliser), as a Python int."""
+    f = _L().haste_oracle_rewire_mix
+    f.restype = ctypes.c_uint64
+    f.argtypes = [ctypes.c_uint64, ctypes.c_uint64]
+    return int(f(seed & 0xFFFFFFFFFFFFFFFF, counter & 0xFFFFFFFFFFFFFFFF))
+
+
+def rewire(idx, W, G, d, rho, init_random=False, seed=0, resort=True, momentum=None):
+    """Algorithm 3, group-shared rewiring (readings in oracle/haste_oracle.cpp).  Returns a dict with
+    the new idx [NG,K] int32, W [L,K] float32 (random weights NOT yet rounded to a storage type), momentum (or None),
+    the fp32 scores [NG,K], the mask [NG,K] (uint8) and m."""
+    idx = np.array(idx, dtype=np.int32, order="C", copy=True)
+    W = np.array(W, dtype=np.float32, order="C", copy=True)
+    L, K = W.shape
+    NG = idx.shape[0]
+    assert NG == -(-L // G) and idx.shape[1] == K
+    mom = None if momentum is None else np.array(momentum, dtype=np.float32, order="C", copy=True)
+    scores = np.empty((NG, K), dtype=np.float32)
+    mask = np.empty((NG, K), dtype=np.uint8)
+    f = _L().haste_oracle_rewire
+    f.restype = ctypes.c_int64
+    m = f(ctypes.c_int64(L), ctypes.c_int(G), ctypes.c_int(K), ctypes.c_int(d), _p(idx), _p(W), _p(mom), ctypes.c_double(rho),
+          ctypes.c_int(1 if init_random else 0), ctypes.c_uint64(seed), ctypes.c_int(1 if resort else 0), _p(scores), _p(mask))
+    if m < 0:
+        raise ValueError("oracle.rewire failed")
+    return dict(idx=idx, W=W, momentum=mom, scores=scores, mask=mask, m=int(m))

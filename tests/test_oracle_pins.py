@@ -361,3 +361,78 @@ def test_sgd_momentum_closed_forms(oracle):
     assert abs(v1[0] - 1.42) < 1e-15 and abs(w1[0] - 1.858) < 1e-15
     # the sign of the step: a positive gradient lowers the weight
     assert oracle.sgd_momentum(np.array([0.0]), np.array([1.0]), np.array([0.0]), 1.0, 0.5)[0][0] == -1.0
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Algorithm 3, group-shared rewiring
+# ------------------------------------------------------------------------------------------------------------------
+def test_rewire_generator_is_splitmix64(oracle):
+    # SplitMix64 seeded with 0: the published first outputs of the reference generator (state += golden ratio, then mix)
+    assert oracle.rewire_mix(0, 0) == 0xE220A8397B1DCDAF
+    assert oracle.rewire_mix(0, 1) == 0x6E789E6AA1B965F4
+    assert oracle.rewire_mix(0, 2) == 0x06C45D188009454F
+
+
+def _rw_case(seed, L, G, K, d, w_std=0.3):
+    inp = synth.small_case(seed, 4, d, L, G, K, dtype="f32", w_std=w_std, with_bias=False)
+    return inp
+
+
+@pytest.mark.parametrize("L,G,K,d", [(64 * 5 + 7, 64, 16, 40), (37, 8, 8, 24), (16 * 9, 16, 32, 64)])
+def test_rewire_properties(oracle, L, G, K, d):
+    inp = _rw_case(3, L, G, K, d)
+    NG = -(-L // G)
+    rho = 0.2
+    out = oracle.rewire(inp.idx, inp.W, G, d, rho, init_random=False, seed=77, resort=False)
+    m = int(np.floor(NG * K * rho))
+    assert out["m"] == m and int(out["mask"].sum()) == m                       # exactly floor(NG K rho) slots
+    # scores: the mean of |w| over the group's labels, against numpy in fp64 -- the fp32 order of additions moves
+    # a score by a few ulp, it cannot move it further
+    for k in range(NG):
+        rows = inp.W[k * G:min(L, (k + 1) * G)]
+        assert np.allclose(out["scores"][k], np.abs(rows.astype(np.float64)).mean(axis=0), rtol=1e-5, atol=0)
+    # the mask holds the m smallest: nothing left out is smaller than anything taken
+    S, M = out["scores"].ravel(), out["mask"].ravel().astype(bool)
+    assert S[M].max() <= S[~M].min()
+    # untouched slots keep idx and weights; touched slots: idx in range, weights zero for EVERY label of the group
+    keep = ~out["mask"].astype(bool)
+    assert np.array_equal(out["idx"][keep], inp.idx[keep])
+    assert np.all((out["idx"] >= 0) & (out["idx"] < d))
+    lab_mask = np.repeat(out["mask"], G, axis=0)[:L].astype(bool)
+    assert np.all(out["W"][lab_mask] == 0) and np.array_equal(out["W"][~lab_mask], inp.W[~lab_mask])
+    # the regrown feature is floor(d * h / 2^64) of the generator's word for that slot (Unif{0..H-1})
+    for k, j in np.argwhere(out["mask"])[:20]:
+        h = oracle.rewire_mix(77, int(k) * K + int(j))
+        assert out["idx"][k, j] == (h * d) >> 64
+    # zero-initialised slots contribute nothing: the layer computes what the old one computed with those weights zeroed
+    z_new = oracle.tail_forward(inp.X, out["idx"], out["W"], None, inp.rowptr, inp.col, G)["z"]
+    z_old = oracle.tail_forward(inp.X, inp.idx, np.where(lab_mask, 0.0, inp.W).astype(np.float32), None, inp.rowptr, inp.col, G)["z"]
+    assert np.allclose(z_new, z_old, rtol=0, atol=1e-12)
+    # rho = 0: nothing happens
+    out0 = oracle.rewire(inp.idx, inp.W, G, d, 0.0)
+    assert out0["m"] == 0 and np.array_equal(out0["idx"], inp.idx) and np.array_equal(out0["W"], inp.W)
+
+
+def test_rewire_random_init_and_resort(oracle):
+    L, G, K, d = 64 * 4 + 9, 64, 32, 200
+    inp = _rw_case(5, L, G, K, d)
+    mom = np.ones((L, K), dtype=np.float32)
+    a = oracle.rewire(inp.idx, inp.W, G, d, 0.3, init_random=True, seed=9, resort=False, momentum=mom)
+    b = oracle.rewire(inp.idx, inp.W, G, d, 0.3, init_random=True, seed=9, resort=True, momentum=mom)
+    lab_mask = np.repeat(a["mask"], G, axis=0)[:L].astype(bool)
+    r = 1.0 / np.sqrt(K)
+    w = a["W"][lab_mask]
+    assert np.all(np.abs(w) <= r) and abs(w.mean()) < 0.1 * r and w.std() > 0.4 * r   # Unif(-1/sqrt(F), 1/sqrt(F))
+    assert np.all(a["momentum"][lab_mask] == 0) and np.all(a["momentum"][~lab_mask] == 1)
+    # resort: every touched row ascending, same multiset of (feature, weight column) pairs, same function (pin P8)
+    touched = a["mask"].any(axis=1)
+    assert np.all(np.diff(b["idx"][touched], axis=1) >= 0)
+    assert np.array_equal(np.sort(a["idx"], axis=1), np.sort(b["idx"], axis=1))
+    za = oracle.tail_forward(inp.X, a["idx"], a["W"], None, inp.rowptr, inp.col, G)["z"]
+    zb = oracle.tail_forward(inp.X, b["idx"], b["W"], None, inp.rowptr, inp.col, G)["z"]
+    assert np.allclose(za, zb, rtol=0, atol=1e-12)
+    assert np.array_equal(b["idx"][~touched], inp.idx[~touched])
+    # ties: with all-equal scores the flat index decides -- the first m slots go
+    Wc = np.full((L, K), 0.25, dtype=np.float32)
+    t = oracle.rewire(inp.idx, Wc, G, d, 0.1, resort=False)
+    assert np.array_equal(np.flatnonzero(t["mask"].ravel()), np.arange(t["m"]))
