@@ -158,6 +158,20 @@ int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* id
                        float* momentum, float* bias, float* bias_momentum, float lr, float mu, float weight_decay,
                        float* dX, int accumulate_dX, void* stream);
 
+/* Group-shared rewiring, Algorithm 3 of the paper; readings in DESIGN.md R15.
+ *   scores S[k,j] = mean over the labels l of group k of |W[l,j]|   (fp32, labels in ascending order)
+ *   the m = floor(NG K rho) smallest entries of S are pruned        (ties: smaller k K + j first)
+ *   pruned slot: idx[k,j] <- Unif{0..d-1}; W[l,j] <- 0 (init_random = 0) or Unif(-1/sqrt(K), 1/sqrt(K)) (init_random = 1)
+ *   for every label l of group k; momentum[l,j] <- 0 if a momentum buffer is given.
+ * Random numbers come from a counter-based generator keyed by `seed` (SplitMix64; the result does not depend on the launch).
+ * resort != 0: every touched idx row is re-sorted ascending (stable) and the W (and momentum) columns of its labels are
+ * permuted with it -- the layer's function does not change, and sorted rows keep the fast path of the dX kernel.
+ * Regrowth may duplicate a feature inside a row (the paper does not de-duplicate either): every kernel here handles that.
+ * idx [NG,K] int32, W [L,K] dtype, momentum [L,K] fp32 or NULL: device memory, updated in place.  *n_pruned (host, may be
+ * NULL) receives m.  Any G, K <= 3000, both dtypes.  Asynchronous on `stream`. */
+int haste_rewire(haste_layer_t* h, int32_t* idx, void* W, float* momentum, float rho, int init_random, uint64_t seed,
+                 int resort, int64_t* n_pruned, void* stream);
+
 /* dY layout helpers: library layout <-> plain [B,L] row-major fp32. */
 int haste_dy_unpack(const haste_layer_t* h, int B, const void* dY, float* out_BL, void* stream);
 int haste_dy_pack(const haste_layer_t* h, int B, const float* in_BL, void* dY, void* stream);

@@ -1,5 +1,6 @@
 // haste_api.cu -- the C-ABI boundary (include/haste.h): handles, argument checks,
 // workspace, kernel-family dispatch.  No arithmetic of the method lives here.
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -92,6 +93,7 @@ struct haste_layer {
   float* partials;  // [n_partials] per-CTA loss partials (tcgen05 family)
   int n_partials;
   int* flag;        // validate_index result
+  void* rw_ws;      // rewiring workspace (scores, mask, ...; allocated on first use)
   float* topk_val;  // fused top-k candidates [num_SMs][4 sets][128][8] (allocated on first use)
   int* topk_idx;
   TcTailState* tc;  // tcgen05 family state (tensor maps, counters) or NULL
@@ -218,7 +220,7 @@ int haste_destroy(haste_layer_t* h) {
   DeviceGuard guard(h->device);
   if (h->tc) tc_tail_destroy(h->tc);
   if (h->prof) { h->prof->destroy(); delete h->prof; }
-  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->dx_part); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag); cudaFree(h->topk_val); cudaFree(h->topk_idx);
+  cudaFree(h->Xt); cudaFree(h->dXt); cudaFree(h->dx_part); cudaFree(h->loss_acc); cudaFree(h->partials); cudaFree(h->flag); cudaFree(h->topk_val); cudaFree(h->topk_idx); cudaFree(h->rw_ws);
   delete h;
   return HASTE_OK;
 }
@@ -520,6 +522,27 @@ int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* id
   h->last_launches += n;
   pf.end(HASTE_KERNEL_DW, st);
   return HASTE_OK;
+}
+
+int haste_rewire(haste_layer_t* h, int32_t* idx, void* W, float* momentum, float rho, int init_random, uint64_t seed, int resort,
+                 int64_t* n_pruned, void* stream) {
+  if (n_pruned) *n_pruned = 0;
+  if (!h || !idx || !W) { set_error("haste_rewire: handle, idx and W are required"); return HASTE_ERR_INVALID_ARG; }
+  if (!(rho >= 0.f && rho <= 1.f)) { set_error("haste_rewire: rho must be in [0, 1]"); return HASTE_ERR_INVALID_ARG; }
+  DeviceGuard guard(h->device);
+  const int64_t n = h->NG * h->cfg.K;
+  const int64_t m = (int64_t)std::floor((double)n * (double)rho);
+  if (n_pruned) *n_pruned = m;
+  if (m <= 0) return HASTE_OK;
+  if (!h->rw_ws && cudaMalloc(&h->rw_ws, rewire_workspace_bytes(h->NG, h->cfg.K)) != cudaSuccess) {
+    set_error("haste_rewire: workspace allocation failed");
+    return HASTE_ERR_NOMEM;
+  }
+  int rc = launch_rewire(h->cfg.dtype, idx, W, momentum, h->cfg.L, h->cfg.G, h->cfg.K, h->cfg.d, m, init_random ? 1 : 0, seed,
+                         resort ? 1 : 0, h->rw_ws, (cudaStream_t)stream);
+  if (rc == HASTE_ERR_UNSUPPORTED) set_error("haste_rewire: shape not supported (K <= 3000)");
+  h->last_launches = 5;
+  return rc;
 }
 
 int haste_set_profiling(haste_layer_t* h, int depth) {

@@ -19,6 +19,11 @@ int launch_dy_unpack(haste_dtype_t dt, const void* dY, float* out_BL, int B, int
 int launch_dy_pack(haste_dtype_t dt, const float* in_BL, void* dY, int B, int64_t L, int G, cudaStream_t st);
 int launch_validate_index(const int32_t* idx, int64_t NG, int K, int d, int check_sorted, int* flag, cudaStream_t st);
 
+// ---- Algorithm 3, group-shared rewiring (rewire.cu): any G, K, dtype; ws = rewire_workspace_bytes(NG, K) bytes of device memory
+size_t rewire_workspace_bytes(int64_t NG, int K);
+int launch_rewire(haste_dtype_t dt, int32_t* idx, void* W, float* mom, int64_t L, int G, int K, int d, int64_t m, int init_random,
+                  uint64_t seed, int resort, void* ws, cudaStream_t st);
+
 // ---- generic CUDA-core family (simt_kernels.cu): any G, K, d; fp32 or bf16 storage ----
 int launch_simt_forward(haste_dtype_t dt, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W,
                         const float* bias, const int32_t* rowptr, const int32_t* col, double* loss_acc, void* dY,

@@ -21,7 +21,7 @@ HASTE_OK, HASTE_ERR_INVALID_ARG, HASTE_ERR_BAD_INDEX, HASTE_ERR_UNSUPPORTED, HAS
 # Every symbol include/haste.h declares (tests check the library exports all of them).
 SYMBOLS = [
     "haste_create", "haste_destroy", "haste_dy_bytes", "haste_validate_index", "haste_forward_loss", "haste_forward_logits", "haste_forward_topk",
-    "haste_backward", "haste_backward_sgd", "haste_dy_unpack", "haste_dy_pack", "haste_head_create", "haste_head_destroy",
+    "haste_backward", "haste_backward_sgd", "haste_rewire", "haste_dy_unpack", "haste_dy_pack", "haste_head_create", "haste_head_destroy",
     "haste_head_forward_loss", "haste_head_backward", "haste_status_string", "haste_last_error",
     "haste_kernel_family", "haste_head_kernel_family", "haste_last_launch_count", "haste_head_last_launch_count",
     "haste_set_profiling", "haste_kernel_ms", "haste_head_set_profiling", "haste_head_kernel_ms",
@@ -66,6 +66,7 @@ def lib():
     L.haste_forward_topk.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]
     L.haste_backward.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     L.haste_backward_sgd.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, vp, i32, vp]
+    L.haste_rewire.argtypes = [vp, vp, vp, vp, f32, i32, ctypes.c_uint64, i32, ctypes.POINTER(ctypes.c_int64), vp]
     L.haste_dy_unpack.argtypes = [vp, i32, vp, vp, vp]
     L.haste_dy_pack.argtypes = [vp, i32, vp, vp, vp]
     L.haste_head_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int32, i64, ctypes.c_int32, i32, i64, f32, u32, i32]
@@ -180,6 +181,13 @@ class HasteLayer:
         _check(lib().haste_backward_sgd(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(dY), _ptr(momentum), _ptr(bias),
                                         _ptr(bias_momentum), lr, mu, weight_decay, _ptr(dX), 1 if accumulate_dX else 0,
                                         _stream(stream)))
+
+    def rewire(self, idx, W, rho, momentum=None, init_random=False, seed=0, resort=True, stream=None):
+        """Algorithm 3 in place on idx / W / momentum; returns the number of pruned slots."""
+        m = ctypes.c_int64(0)
+        _check(lib().haste_rewire(self.h, _ptr(idx), _ptr(W), _ptr(momentum), rho, 1 if init_random else 0, seed,
+                                  1 if resort else 0, ctypes.byref(m), _stream(stream)))
+        return m.value
 
     def dy_unpack(self, B, dY, out_BL, stream=None):
         _check(lib().haste_dy_unpack(self.h, B, _ptr(dY), _ptr(out_BL), _stream(stream)))
