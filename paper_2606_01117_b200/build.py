@@ -17,7 +17,6 @@ OBJ = os.path.join(_DIR, "build")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr",
-] + os.environ.get("HASTE_NVCC_EXTRA", "").split() + [
 ]
 
 
