@@ -506,6 +506,38 @@ def main():
                        "dense_bottleneck_note": "torch.matmul [B,%d] x [L,%d]^T -> [B,L] in %s (cuBLAS), same FLOPs and W/output bytes, no gather" % (K, K, cfg.dtype)}
         del Zb, Hb, Wp
         layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY)     # dY holds dY again for what follows
+    # ---- the round-2 calls beside the step (not part of `value`): the SGD-momentum step fused into the dW kernel
+    # (haste_backward_sgd, dX skipped here) and the fused top-k forward (haste_forward_topk, k = 5, forward + merge)
+    extras = None
+    if rank == 0 and layer.kernel_family == 1 and cfg.dtype == "bf16":
+        extras = {}
+        nx = min(args.steps, nprof, 20)
+        try:
+            W2, mom = W.clone(), torch.zeros(L, K, device=dev)
+            for _ in range(2):
+                layer.backward_sgd(B, X, idx, W2, dY, mom, 0.01, 0.9)
+            torch.cuda.synchronize()
+            for _ in range(nx):
+                layer.backward_sgd(B, X, idx, W2, dY, mom, 0.01, 0.9)
+            torch.cuda.synchronize()
+            t = [layer.kernel_ms(haste.KERNEL_DW, a) for a in range(nx)]
+            sb = cfg.NG * G * B * esz + cfg.NG * K * 4 + B * d * esz + 2 * L * K * esz + 2 * L * K * 4
+            g = sb / (float(np.mean(t)) * 1e-3) / 1e9
+            extras["dW_sgd_fused"] = {"ms": float(np.mean(t)), "ms_median": float(np.median(t)), "ms_min": float(np.min(t)), "alg_bytes": int(sb),
+                                      "GB/s": g, "frac_hbm": g / _peaks()["hbm"], "note": "dW never written; W (bf16) and momentum (fp32) read and written in place"}
+            del W2, mom
+        except haste.HasteError as e:
+            extras["dW_sgd_fused"] = {"unsupported": str(e)}
+        tv, ti = torch.empty(B, 5, device=dev), torch.empty(B, 5, dtype=torch.int64, device=dev)
+        for _ in range(2):
+            layer.forward_topk(B, X, idx, W, None, 5, tv, ti)
+        torch.cuda.synchronize()
+        for _ in range(nx):
+            layer.forward_topk(B, X, idx, W, None, 5, tv, ti)
+        torch.cuda.synchronize()
+        t = [layer.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nx)]
+        extras["forward_topk_k5"] = {"ms": float(np.mean(t)), "ms_median": float(np.median(t)), "ms_min": float(np.min(t)),
+                                     "note": "forward kernel with per-thread candidate lists + merge kernel; no [B,L] buffer"}
     layer.set_profiling(0)
     if use_head:
         head.set_profiling(0)
@@ -588,6 +620,8 @@ def main():
                           "note": "the same K steps repeated with the library's per-kernel CUDA events on; `kernels` and `roofline` come from this pass, `value` does not"},
         "loss": [float(v) for v in loss.cpu().tolist()],
     }
+    if extras:
+        out["extras"] = extras
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(cfg)
     print(json.dumps(out))

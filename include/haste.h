@@ -29,10 +29,11 @@
  *  - Every function returns a haste_status_t; 0 is success.  Nothing throws, aborts
  *    or prints.  Argument errors are detected on the host before any launch.
  *    Index CONTENTS are not checked by the hot calls; haste_validate_index does it.
- *  - Pointers to X, W, dY, dW must be 16-byte aligned.
+ *  - Pointers to X, W, idx, dY, dW (and Z, momentum) must be 16-byte aligned.
  *  - idx rows may hold any values in [0,d): duplicates add, order is free
  *    (reading R4).  HASTE_IDX_SORTED_DISTINCT is a caller's promise that
- *    only enables faster paths.
+ *    haste_validate_index checks; no kernel relies on it (the dX kernel tests every
+ *    row itself and sends a row that is not strictly ascending down its atomic path).
  *  - Targets: one CSR over GLOBAL label ids, ascending and distinct within a row;
  *    a layer looks only at ids in [label_offset, label_offset + L).
  *  - dY of the sparse tail lives in a library-defined layout (group-blocked:

@@ -148,11 +148,17 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
     return HASTE_ERR_INVALID_ARG;
   }
   if (cfg->G > 1024 || cfg->K > 4096) {
-    set_error("haste_create: G <= 1024 and K <= 4096 are supported");
+    set_error("haste_create: G <= 1024 and K <= 1700 are supported");
     return HASTE_ERR_UNSUPPORTED;
   }
   const int64_t NG = (cfg->L + cfg->G - 1) / cfg->G;
   if (NG > 0x7fffffffLL) { set_error("haste_create: too many groups"); return HASTE_ERR_UNSUPPORTED; }
+  // limits of the generic CUDA-core family, checked here so that no hot call fails at launch time: its forward stages
+  // K x 33 words of shared memory per block (227 KB at most), and its grids put ceil(B/32) into gridDim.y
+  if (cfg->K > 1700 || cfg->B_max > 65535 * 32) {
+    set_error("haste_create: K <= 1700 and B_max <= 2 097 120 are supported");
+    return HASTE_ERR_UNSUPPORTED;
+  }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
     cudaGetLastError();
@@ -582,6 +588,11 @@ int haste_head_create(haste_head_t** out, int32_t d, int64_t L_h, int32_t B_max,
   if (d <= 0 || L_h < 0 || B_max <= 0 || L_h > 0x7fffffffLL || (dtype != HASTE_F32 && dtype != HASTE_BF16)) {
     set_error("haste_head_create: bad sizes or dtype");
     return HASTE_ERR_INVALID_ARG;
+  }
+  // grids of the generic CUDA-core head kernels put ceil(L_h/64) and ceil(B/64) into gridDim.y
+  if (L_h > 65535LL * 64 || B_max > 65535 * 64) {
+    set_error("haste_head_create: L_h <= 4 194 240 and B_max <= 4 194 240 are supported");
+    return HASTE_ERR_UNSUPPORTED;
   }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
