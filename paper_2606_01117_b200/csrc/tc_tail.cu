@@ -338,21 +338,25 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
               }
               if (jj >= nvalid) z[j] = -INFINITY;
             }
-            const float m = max3(max3(z[0], z[1], z[2]), max3(z[3], z[4], z[5]), fmaxf(z[6], z[7]));
-            if (m > tv[KL - 1]) {
-              const int l0 = (int)(g * G) + sc * 32 + r8 * 8;
+            float m = max3(max3(z[0], z[1], z[2]), max3(z[3], z[4], z[5]), fmaxf(z[6], z[7]));
+            // A run that holds a candidate for SOME lane is entered by the whole warp (early in a stripe: most runs), so
+            // what happens inside must be short: pull out the run's maximum, insert it, knock it out, look again -- one
+            // pass per candidate of the lane that has most (usually one), not one branch per logit.
+            const int l0 = (int)(g * G) + sc * 32 + r8 * 8;
+            while (m > tv[KL - 1]) {
+              int js = 7;
 #pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                if (z[j] > tv[KL - 1]) {             // insert into the descending list (stable: earlier labels win ties)
-                  tv[KL - 1] = z[j]; ti[KL - 1] = l0 + j;
+              for (int j = 6; j >= 0; --j) js = z[j] == m ? j : js;      // first position of the maximum: earlier labels win ties
+              tv[KL - 1] = m; ti[KL - 1] = l0 + js;
 #pragma unroll
-                  for (int i = KL - 1; i > 0; --i)
-                    if (tv[i] > tv[i - 1]) {
-                      const float a = tv[i]; tv[i] = tv[i - 1]; tv[i - 1] = a;
-                      const int b_ = ti[i]; ti[i] = ti[i - 1]; ti[i - 1] = b_;
-                    }
+              for (int i = KL - 1; i > 0; --i)
+                if (tv[i] > tv[i - 1]) {
+                  const float a = tv[i]; tv[i] = tv[i - 1]; tv[i - 1] = a;
+                  const int b_ = ti[i]; ti[i] = ti[i - 1]; ti[i - 1] = b_;
                 }
-              }
+#pragma unroll
+              for (int j = 0; j < 8; ++j) z[j] = j == js ? -INFINITY : z[j];
+              m = max3(max3(z[0], z[1], z[2]), max3(z[3], z[4], z[5]), fmaxf(z[6], z[7]));
             }
           }
         } else if constexpr (TOPK < 0) {    // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
