@@ -124,20 +124,36 @@ __global__ void topk_merge_kernel(const float* __restrict__ cv, const int* __res
   int ti[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) { tv[i] = -INFINITY; ti[i] = 0x7fffffff; }
-  for (int e = lane; e < total; e += 32) {
-    const int s = e / per_cta, w = e - s * per_cta;
-    const int set = ntp == 2 ? 2 * (w >> 3) + (bt & 1) : (w >> 3);
-    const size_t o = ((((size_t)s * NP + pr) * NSET + set) * 128 + r) * 8 + (w & 7);
-    const float z = cv[o];
-    const int l = ci[o];
-    if (l >= 0 && (z > tv[7] || (z == tv[7] && l < ti[7]))) {
-      tv[7] = z; ti[7] = l;
+  // 8 candidates per lane at a time: their loads are in flight together (one by one the scan is a chain of L2 round trips:
+  // 42 us for 512 rows), then they are inserted in order
+  for (int e0 = lane; e0 < total; e0 += 32 * 8) {
+    float zc[8];
+    int lc[8];
 #pragma unroll
-      for (int i = 7; i > 0; --i)
-        if (tv[i] > tv[i - 1] || (tv[i] == tv[i - 1] && ti[i] < ti[i - 1])) {
-          const float a = tv[i]; tv[i] = tv[i - 1]; tv[i - 1] = a;
-          const int c = ti[i]; ti[i] = ti[i - 1]; ti[i - 1] = c;
-        }
+    for (int u = 0; u < 8; ++u) {
+      const int e = e0 + 32 * u;
+      zc[u] = -INFINITY; lc[u] = -1;
+      if (e < total) {
+        const int s = e / per_cta, w = e - s * per_cta;
+        const int set = ntp == 2 ? 2 * (w >> 3) + (bt & 1) : (w >> 3);
+        const size_t o = ((((size_t)s * NP + pr) * NSET + set) * 128 + r) * 8 + (w & 7);
+        zc[u] = __ldcg(cv + o);
+        lc[u] = __ldcg(ci + o);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const float z = zc[u];
+      const int l = lc[u];
+      if (l >= 0 && (z > tv[7] || (z == tv[7] && l < ti[7]))) {
+        tv[7] = z; ti[7] = l;
+#pragma unroll
+        for (int i = 7; i > 0; --i)
+          if (tv[i] > tv[i - 1] || (tv[i] == tv[i - 1] && ti[i] < ti[i - 1])) {
+            const float a = tv[i]; tv[i] = tv[i - 1]; tv[i - 1] = a;
+            const int c = ti[i]; ti[i] = ti[i - 1]; ti[i - 1] = c;
+          }
+      }
     }
   }
   for (int round = 0; round < k; ++round) {
