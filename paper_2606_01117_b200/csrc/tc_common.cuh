@@ -168,6 +168,19 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
       : "r"(taddr)
       : "memory");
 }
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
+}
+// the first N (8, 16 or 32) entries of v: N consecutive columns (narrow groups, G < 32, have narrow accumulators)
+template <int N> __device__ __forceinline__ void tmem_ld_first(uint32_t taddr, uint32_t (&v)[32]) {
+  static_assert(N == 8 || N == 16 || N == 32, "tmem_ld_first");
+  if constexpr (N == 32) tmem_ld32(taddr, v);
+  else if constexpr (N == 16) tmem_ld16(taddr, reinterpret_cast<uint32_t(&)[16]>(v[0]));
+  else tmem_ld8(taddr, reinterpret_cast<uint32_t(&)[8]>(v[0]));
+}
 
 // Shared-memory matrix descriptor (sm_100 format): start address, leading / stride byte offsets (all >> 4),
 // version 1 at bits [46,48), layout type at bits [61,64) (2 = 128-byte swizzle).
@@ -188,6 +201,16 @@ __device__ __forceinline__ uint64_t make_sdesc_sw64(uint32_t saddr, uint32_t lbo
   d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
   d |= (uint64_t)1 << 46;
   d |= (uint64_t)4 << 61;
+  return d;
+}
+// Same with the 32-byte swizzle (layout type 6): rows of 32 B (16 bf16), atoms of 8 rows x 32 B, 256-B aligned.
+__device__ __forceinline__ uint64_t make_sdesc_sw32(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)6 << 61;
   return d;
 }
 // Instruction descriptor, kind::f16: bf16 x bf16 -> fp32, M x N, operand majors (0 = K-major, 1 = MN-major).

@@ -42,8 +42,16 @@ template <int G, int K, bool F32, bool SGD = false> struct DwCfg {
   // G = 32: two consecutive groups form one virtual group of GV = 64 labels and KV = 2K slots (their idx rows are
   // adjacent in memory, so are their labels).  D [64 x 2K] then holds dW_g in rows 0-31 x columns [0,K) and dW_{g+1}
   // in rows 32-63 x columns [K,2K); the off-diagonal blocks are computed and ignored (the tensor pipe has the room).
-  static constexpr bool PAIR = G == 32;
-  static constexpr int GV = PAIR ? 64 : G;                  // MMA M
+  // G < 64 otherwise (G = 32 with K = 128, whose pair would need N = 264; G = 16; G = 8): the MMA is still M = 64, but only
+  // its first G label rows are real -- the A descriptor walks on into whatever follows the dY image, and accumulator
+  // rows G .. 63 are never read (rows of D are independent).  The tensor pipe has the room: what bounds a narrow group
+  // is the gather of its K feature rows, which G labels share instead of 64.  G = 8: the TMA box is 16 labels wide over
+  // a tensor that has 8, so labels 8-15 of every row arrive as zeros and the image is the G = 16 one.
+  static constexpr bool PAIR = G == 32 && K == 64;
+  static constexpr bool PADM = G < 64 && !PAIR;
+  static constexpr int GL = PAIR ? 64 : G;                  // labels per (virtual) group
+  static constexpr int GV = G < 64 ? 64 : G;                // MMA M
+  static constexpr int YROW = PADM ? (G >= 32 ? 64 : 32) : (PAIR ? 64 : 128);   // bytes per batch row of the dY image
   static constexpr int KV = PAIR ? 2 * K : K;               // gathered slots per (virtual) group
   static constexpr int NE = GV == 128 ? 16 : 8;             // rows of ones appended to the H image
   static constexpr int N = KV + NE;                         // MMA N
@@ -52,7 +60,7 @@ template <int G, int K, bool F32, bool SGD = false> struct DwCfg {
   // pays one barrier wait and one commit per 8 MMAs (with 64-row k-blocks its ~0.3 us loop overhead per k-block
   // was the kernel's bottleneck)
   static constexpr int HH_BYTES = (KV + 16) * 128;          // one half of the H image, multiple of 1024
-  static constexpr int YH_BYTES = GV * 128;                 // one half of the dY image: [G/64 atoms][64 rows][128 B]; PAIR: [2 groups][64 rows][64 B]
+  static constexpr int YH_BYTES = PADM ? 64 * YROW : GV * 128;   // one half of the dY image: [G/64 atoms][64 rows][128 B]; PAIR: [2 groups][64 rows][64 B]; PADM: [64 rows][YROW]
   static constexpr int H_BYTES = 2 * HH_BYTES;
   static constexpr int Y_BYTES = 2 * YH_BYTES;
   static constexpr int STAGE = H_BYTES + Y_BYTES;
@@ -176,7 +184,11 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     constexpr uint32_t idesc = make_idesc_bf16(C::GV, C::N, /*A (dY) MN-major*/ 1, /*B (H^T) K-major*/ 0);
     const uint64_t bdesc0 = make_sdesc_sw128(sbase, 16, 1024);
     // A = the dY k-block as stored, MN-major: atoms of 64 labels x 128 B rows, or (PAIR) two groups of 32 labels x 64 B rows
-    const uint64_t adesc0 = C::PAIR ? make_sdesc_sw64(sbase + C::H_BYTES, 4096, 512) : make_sdesc_sw128(sbase + C::H_BYTES, 8192, 1024);
+    // PADM: one real atom of 32 (16) labels; the atoms after it are read from the bytes that follow (leading offset 2048 / 512)
+    const uint64_t adesc0 = C::PAIR ? make_sdesc_sw64(sbase + C::H_BYTES, 4096, 512)
+                          : !C::PADM ? make_sdesc_sw128(sbase + C::H_BYTES, 8192, 1024)
+                          : C::YROW == 64 ? make_sdesc_sw64(sbase + C::H_BYTES, 2048, 512)
+                                          : make_sdesc_sw32(sbase + C::H_BYTES, 512, 256);
     int it = 0;
     for (int i = 0; i < n_my; ++i) {
       const int slot = i & 1;
@@ -191,7 +203,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
-            const uint64_t ad = adesc0 + so + (uint64_t)(((j >> 2) * C::YH_BYTES + (j & 3) * (C::PAIR ? 1024 : 2048)) >> 4);
+            const uint64_t ad = adesc0 + so + (uint64_t)(((j >> 2) * C::YH_BYTES + (j & 3) * (16 * C::YROW)) >> 4);
             const uint64_t bd = bdesc0 + so + (uint64_t)(((j >> 2) * C::HH_BYTES + (j & 3) * 32) >> 4);
             umma_f16(d, ad, bd, idesc, (kb | j) ? 1u : 0u);
           }
@@ -214,7 +226,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
 #pragma unroll
           for (int hf = 0; hf < 2; ++hf)
 #pragma unroll
-            for (int a = 0; a < C::GV / 64 + (C::PAIR ? 1 : 0); ++a) {
+            for (int a = 0; a < (C::PADM ? 1 : C::GV / 64 + (C::PAIR ? 1 : 0)); ++a) {
               uint8_t* dst = smem + st * C::STAGE + C::H_BYTES + hf * C::YH_BYTES + a * (C::PAIR ? 4096 : 8192);
               if (C::PAIR) tma_load_3d(dst, &tmY, &full[st], 0, kb * 128 + hf * 64, (int)(2 * g + a));   // group 2v+a (zero-filled past NG)
               else tma_load_3d(dst, &tmY, &full[st], a * 64, kb * 128 + hf * 64, (int)g);
@@ -228,11 +240,20 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     const uint32_t sbuf0 = sbase + C::OFF_EPI + q * 4096;
     const uint32_t swz = (uint32_t)(lane & 7);
     int nstore = 0;
+    // label rows of this warp that are real: M = 64 puts rows 16 q .. 16 q + 15 into lanes 0-15 of quadrant q
+    constexpr int RWC = C::RW;
+    const int rwv = C::PADM ? max(0, min(RWC, G - RWC * q)) : RWC;
     for (int i = 0; i < n_my; ++i) {
       const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
       const int slot = i & 1;
       mbar_wait(&t_full[slot], (i >> 1) & 1);
       tc_fence_after();
+      if (rwv == 0) {                     // (PADM) a quadrant past the group's labels: keep step with the others, nothing to do
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&t_empty[slot]);
+        continue;
+      }
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * C::TS;
       const uint32_t tcol = taddr + (C::PAIR && q >= 2 ? K : 0);   // PAIR: quadrants 2, 3 hold group 2v+1, whose dW sits in columns [K, 2K)
       if constexpr (SGD) {
@@ -241,13 +262,13 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
         // dW store), and the warp then walks them in memory order -- 8 lanes per label row, 16 bytes of momentum and 8 of
         // W each -- so that every global access is a run of whole 128-byte lines and all of a pass's loads are in flight
         // together.  The next group's rows are pulled into L2 meanwhile.
-        const int64_t l0 = g * C::GV + q * C::RW;                    // first label row of this warp
+        const int64_t l0 = g * C::GL + q * C::RW;                    // first label row of this warp
         const int64_t l = l0 + lane;
-        const bool own = lane < C::RW && l < p.L;
+        const bool own = lane < rwv && l < p.L;
         if (i + 1 < n_my) {
-          const int64_t ln0 = l0 + (int64_t)gridDim.x * C::GV;
+          const int64_t ln0 = l0 + (int64_t)gridDim.x * C::GL;
           constexpr int WL = K * 2 / 128, ML = K * 4 / 128;          // 128-byte lines per row of W / of the momentum
-          for (int e = lane; e < C::RW * (WL + ML); e += 32) {
+          for (int e = lane; e < rwv * (WL + ML); e += 32) {
             const int r = e / (WL + ML), b = e - r * (WL + ML);
             if (ln0 + r < p.L) {
               const char* a = b < WL ? reinterpret_cast<const char*>(p.W + (ln0 + r) * K) + b * 128
@@ -275,7 +296,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
               const int e = lane + 32 * (h0 + t), r = e >> 3, c16 = e & 7;
-              ok[t] = l0 + r < p.L;
+              ok[t] = r < rwv && l0 + r < p.L;
               g4[t] = lds128f(sbuf0 + r * 128 + ((c16 ^ (r & 7)) << 4));
               if (ok[t]) {
                 const size_t o = (size_t)(l0 + r) * K + c * 32 + c16 * 4;
@@ -337,7 +358,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
-            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 4096, c * (F32 ? 32 : 64), (int)(g * C::GV + q * C::RW));
+            tma_store_2d(&tmO, smem + C::OFF_EPI + q * 4096, c * (F32 ? 32 : 64), (int)(g * C::GL + q * C::RW));
             bulk_commit();
           }
         }
@@ -345,8 +366,8 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
       if (!SGD && p.dbias) {
         const uint32_t v = tmem_ld1(taddr + C::KV);
         tmem_ld_wait();
-        const int64_t l = g * C::GV + q * C::RW + lane;
-        if (lane < C::RW && l < p.L) p.dbias[l] = __uint_as_float(v);
+        const int64_t l = g * C::GL + q * C::RW + lane;
+        if (lane < rwv && l < p.L) p.dbias[l] = __uint_as_float(v);
       }
       tc_fence_before();
       __syncwarp();
@@ -371,15 +392,16 @@ static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const 
   {
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
     const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
-    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 64, 1};
-    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
+    // G = 8: a box of 16 labels over a row of 8 -- the TMA fills labels 8-15 with zeros
+    const uint32_t box[3] = {(uint32_t)std::min(std::max(G, 16), 64), 64, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, C::PADM ? C::YROW : (G >= 64 ? 128 : 64));
     if (rc) return rc;
   }
   if (dW) {
     const int es = F32 ? 4 : 2;
     const uint64_t dims[2] = {(uint64_t)K, (uint64_t)sh.L};
     const uint64_t str[1] = {(uint64_t)K * es};
-    const uint32_t box[2] = {(uint32_t)(128 / es), (uint32_t)C::RW};
+    const uint32_t box[2] = {(uint32_t)(128 / es), (uint32_t)std::min(C::RW, G)};
     int rc = encode_tmap(&tmO, es, dW, 2, dims, str, box, 128);
     if (rc) return rc;
   } else {
@@ -405,9 +427,10 @@ int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_
   if (sh.G == G_ && sh.K == K_)                                                              \
     return f32 ? launch_dw<G_, K_, true>(s, sh, Xt, idx, dY, dW, dbias, st)                  \
                : launch_dw<G_, K_, false>(s, sh, Xt, idx, dY, dW, dbias, st)
-  HASTE_DW(64, 128); HASTE_DW(64, 64); HASTE_DW(128, 64); HASTE_DW(128, 128); HASTE_DW(32, 64);
+  HASTE_DW(64, 128); HASTE_DW(64, 64); HASTE_DW(128, 64); HASTE_DW(128, 128); HASTE_DW(32, 64); HASTE_DW(32, 128);
+  HASTE_DW(16, 64); HASTE_DW(16, 128); HASTE_DW(8, 64); HASTE_DW(8, 128);
 #undef HASTE_DW
-  return HASTE_ERR_UNSUPPORTED;   // G = 32 with K = 128 (the paired MMA would need N = 264): the caller runs the CUDA-core kernel
+  return HASTE_ERR_UNSUPPORTED;
 }
 
 // the same contraction with the SGD-momentum step of the output layer as its epilogue: W [L,K] (bf16) and
@@ -418,7 +441,8 @@ int tc_tail_dw_sgd(TcTailState* s, const TailShape& sh, const void* Xt, const in
   const DwSgd sgd = {W, mom, bias, bmom, lr, mu, wd};
 #define HASTE_DWS(G_, K_) \
   if (sh.G == G_ && sh.K == K_) return launch_dw<G_, K_, true, true>(s, sh, Xt, idx, dY, nullptr, nullptr, st, &sgd)
-  HASTE_DWS(64, 128); HASTE_DWS(64, 64); HASTE_DWS(128, 64); HASTE_DWS(128, 128); HASTE_DWS(32, 64);
+  HASTE_DWS(64, 128); HASTE_DWS(64, 64); HASTE_DWS(128, 64); HASTE_DWS(128, 128); HASTE_DWS(32, 64); HASTE_DWS(32, 128);
+  HASTE_DWS(16, 64); HASTE_DWS(16, 128); HASTE_DWS(8, 64); HASTE_DWS(8, 128);
 #undef HASTE_DWS
   return HASTE_ERR_UNSUPPORTED;
 }

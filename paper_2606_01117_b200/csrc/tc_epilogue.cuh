@@ -110,13 +110,13 @@ __device__ __forceinline__ void epi8(const uint32_t (&v)[32], uint32_t sbias, ui
 // The exact-enough evaluation of 32 logits (see epi32), ONE copy of the code for every caller: it is rare on a freshly
 // initialised layer, and four inlined copies per call site pushed the forward kernels out of the instruction cache
 // (0.184 -> 0.262 ms).  io: v[32] accumulators in, then R[4], P[4] in/out at 32..39 and out[16] at 40..55 (a call through
-// memory; only this path pays for it).
-static __device__ __noinline__ void epi32_wide(uint32_t* io, uint32_t sbias, int has_bias, uint32_t ymask, int nvalid, float s, float* zout) {
+// memory; only this path pays for it).  nj: how many of the 32 are there (narrow groups: 8 or 16).
+static __device__ __noinline__ void epi32_wide(uint32_t* io, uint32_t sbias, int has_bias, uint32_t ymask, int nvalid, float s, float* zout, int nj) {
   float R[4], P[4];
 #pragma unroll
   for (int k = 0; k < 4; ++k) { R[k] = __uint_as_float(io[32 + k]); P[k] = __uint_as_float(io[36 + k]); }
 #pragma unroll 4
-  for (int j = 0; j < 32; j += 2) {
+  for (int j = 0; j < nj; j += 2) {
     float z0 = __uint_as_float(io[j]), z1 = __uint_as_float(io[j + 1]);
     if (has_bias) {
       float b0, b1;
@@ -158,30 +158,31 @@ static __device__ __noinline__ void epi32_wide(uint32_t* io, uint32_t sbias, int
 // logits are wanted; the decision is then refined per 8 logits (warp-uniform), because the special-case code costs more
 // than the math itself and positives are rare (in the dense head ~70 % of the (warp, 128-label tile) pairs hold one).
 // Chains: logit jj feeds P[jj & 3] (and, wide evaluation, R[jj & 3]); pair (j, j+1) = the two lanes of packed chain (j >> 1) & 1.
-template <bool SLOW, bool BIAS>
+// NV: the chunk holds NV = 8, 16 or 32 logits (v[0 .. NV), out[0 .. NV/2)); groups of fewer than 32 labels have NV = G.
+template <bool SLOW, bool BIAS, int NV = 32>
 __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, uint32_t ymask, int nvalid, float s,
                                       float hs, float (&R)[4], float (&P)[4], uint32_t (&out)[16], float* zout) {
   // which evaluation: max |accumulator| over the warp's 32 x 32 logits (+ max |bias| of the 32 labels) against 2.5
   float a4[4] = {0.f, 0.f, 0.f, 0.f};          // four independent chains: one chain of 16 would be ~70 cycles of latency per chunk
 #pragma unroll
-  for (int j = 0; j < 32; j += 2) a4[(j >> 1) & 3] = max3(a4[(j >> 1) & 3], fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1])));
+  for (int j = 0; j < NV; j += 2) a4[(j >> 1) & 3] = max3(a4[(j >> 1) & 3], fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1])));
   float am = max3(fmaxf(a4[0], a4[1]), a4[2], a4[3]);
   if (BIAS) {
-    float b;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(b) : "r"(sbias + (threadIdx.x & 31) * 4));
+    float b = 0.f;
+    if (NV == 32 || (threadIdx.x & 31) < NV) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(b) : "r"(sbias + (threadIdx.x & 31) * 4));
     am += __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fabsf(b))));
   }
   if (__any_sync(0xffffffffu, am > 2.5f)) {
     uint32_t io[56];
 #pragma unroll
-    for (int j = 0; j < 32; ++j) io[j] = v[j];
+    for (int j = 0; j < 32; ++j) io[j] = j < NV ? v[j] : 0u;
 #pragma unroll
     for (int k = 0; k < 4; ++k) { io[32 + k] = __float_as_uint(R[k]); io[36 + k] = __float_as_uint(P[k]); }
-    epi32_wide(io, sbias, BIAS ? 1 : 0, SLOW ? ymask : 0u, SLOW ? nvalid : 32, s, SLOW ? zout : nullptr);
+    epi32_wide(io, sbias, BIAS ? 1 : 0, SLOW ? ymask : 0u, SLOW ? nvalid : NV, s, SLOW ? zout : nullptr, NV);
 #pragma unroll
     for (int k = 0; k < 4; ++k) { R[k] = __uint_as_float(io[32 + k]); P[k] = __uint_as_float(io[36 + k]); }
 #pragma unroll
-    for (int k = 0; k < 16; ++k) out[k] = io[40 + k];
+    for (int k = 0; k < NV / 2; ++k) out[k] = io[40 + k];
     return;
   }
   uint64_t P2[2] = {pk2(P[0], P[1]), pk2(P[2], P[3])};      // (the fast path adds nothing to R: its loss terms are all in P)
@@ -194,7 +195,9 @@ __device__ __forceinline__ void epi32(const uint32_t (&v)[32], uint32_t sbias, u
   } else {                                                                                                           \
     epi8<false, BIAS, J0_>(v, sbias, 0u, 32, s, half2, hs2, P2, out, nullptr);                             \
   }
-  HASTE_EPI8(0) HASTE_EPI8(8) HASTE_EPI8(16) HASTE_EPI8(24)
+  HASTE_EPI8(0)
+  if constexpr (NV > 8) { HASTE_EPI8(8) }
+  if constexpr (NV > 16) { HASTE_EPI8(16) HASTE_EPI8(24) }
 #undef HASTE_EPI8
   upk2(P2[0], P[0], P[1]); upk2(P2[1], P[2], P[3]);
 }

@@ -86,11 +86,17 @@ template <int G, int K> struct FwdCfg {
   static constexpr int NSET = (G == 128 && K == 128) ? 2 : 4;   // epilogue sets (4 warps each); what shared memory allows
   static constexpr int HS = 3;                                  // H stages
   static constexpr int LAG = 1;                                 // producer completion lag (< HS-1, or the MMAs serialise)
+  // narrow groups (G = 16, 8): the MMA is N = GP = 16 wide (the smallest N of an M = 128 MMA); for G = 8 the upper 8 rows
+  // of the W image are never written and the 8 accumulator columns they produce are never read
+  static constexpr int GP = G < 16 ? 16 : G;                    // MMA N = accumulator columns per slot = rows of the W image
+  static constexpr int CW = G < 32 ? G : 32;                    // logits per epilogue chunk
+  static constexpr int NCH = G / CW;                            // chunks per group
   static constexpr int H_BYTES = K * 256;                       // [2 m-blocks][K rows][128 B]
-  static constexpr int W_BYTES = G * K * 2;                     // [K/64 k-blocks][G rows][128 B]
+  static constexpr int W_BYTES = GP * K * 2;                    // [K/64 k-blocks][GP rows][128 B]
+  static constexpr int W_TX = G * K * 2;                        // bytes the TMA box of a group brings
   static constexpr int WS = W_BYTES <= 16384 ? 3 : 2;           // W stages
   static constexpr int ST_BYTES = 128 * (G < 64 ? G : 64) * 2;  // one dY staging tile (<= 64 labels wide) per epilogue set
-  static constexpr int NSLOT = (512 / G) >= 8 ? 8 : (512 / G);  // TMEM accumulator ring (G columns each)
+  static constexpr int NSLOT = (512 / GP) >= 8 ? 8 : (512 / GP);  // TMEM accumulator ring (GP columns each)
   static constexpr int OFF_H = 0;
   static constexpr int OFF_W = OFF_H + HS * H_BYTES;
   static constexpr int OFF_ST = OFF_W + WS * W_BYTES;
@@ -200,7 +206,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     // The whole warp walks the loop and waits; one elected lane issues.  (Issuing from inside `if (lane == 0)` makes
     // ptxas wrap every tcgen05 instruction in an elect/branch loop, and rebuilding both descriptors per MMA is a
     // chain of uniform-datapath ops: together ~1100 cycles per tile, which was this kernel's critical path.)
-    constexpr uint32_t idesc = make_idesc_bf16(128, G, /*A MN-major*/ 1, /*B K-major*/ 0);
+    constexpr uint32_t idesc = make_idesc_bf16(128, C::GP, /*A MN-major*/ 1, /*B K-major*/ 0);
     const uint64_t adesc0 = make_sdesc_sw128(sbase + C::OFF_H, K * 128, 1024);
     const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::OFF_W, 16, 1024);
     for (int T = 0; T < total; ++T) {
@@ -213,10 +219,10 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
       if (elect_one()) {
         const uint64_t ad0 = adesc0 + (uint64_t)((hs * C::H_BYTES) >> 4);       // the address field never carries out
         const uint64_t bd0 = bdesc0 + (uint64_t)((ws * C::W_BYTES) >> 4);
-        const uint32_t d = tmem_base + slot * G;
+        const uint32_t d = tmem_base + slot * C::GP;
 #pragma unroll
         for (int j = 0; j < K / 16; ++j)
-          umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * (G * 128) + (j & 3) * 32) >> 4), idesc,
+          umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * (C::GP * 128) + (j & 3) * 32) >> 4), idesc,
                    j > 0 ? 1u : 0u);
         umma_commit(&h_empty[hs]);
         umma_commit(&t_full[slot]);
@@ -231,10 +237,10 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         const int ws = gl % C::WS;
         const int64_t g = stripe + (int64_t)gl * p.S;
         mbar_wait(&w_empty[ws], ((gl / C::WS) & 1) ^ 1);
-        mbar_arrive_expect_tx(&w_full[ws], C::W_BYTES);
+        mbar_arrive_expect_tx(&w_full[ws], C::W_TX);
 #pragma unroll
         for (int kb = 0; kb < K / 64; ++kb)
-          tma_load_2d(smem + C::OFF_W + ws * C::W_BYTES + kb * (G * 128), &tmW, &w_full[ws], kb * 64, (int)(g * G));
+          tma_load_2d(smem + C::OFF_W + ws * C::W_BYTES + kb * (C::GP * 128), &tmW, &w_full[ws], kb * 64, (int)(g * G));
       }
     }
   } else {
@@ -258,11 +264,13 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     int ti[KL];
 #pragma unroll
     for (int i = 0; i < KL; ++i) { tv[i] = -INFINITY; ti[i] = -1; }
-    // this warp's 32 rows of the half's staging tile(s); rows are 128 B (G >= 64) or 64 B (G = 32)
-    constexpr int ROWB = G >= 64 ? 128 : 64;
+    // this warp's 32 rows of the half's staging tile(s); rows are 128 B (G >= 64) or 2 G bytes (64, 32, 16), swizzled as
+    // the TMA store of that row length expects (none for 16-byte rows)
+    constexpr int CW = C::CW, NCH = C::NCH;
+    constexpr int ROWB = G >= 64 ? 128 : G * 2;
     const uint32_t stage_w = sbase + C::OFF_ST + set * C::ST_BYTES + q * 32 * ROWB;
     const uint32_t stage_row = stage_w + lane * ROWB;
-    const uint32_t swz = G >= 64 ? (uint32_t)(lane & 7) : (uint32_t)((lane >> 1) & 3);
+    const uint32_t swz = G >= 64 ? (uint32_t)(lane & 7) : G == 32 ? (uint32_t)((lane >> 1) & 3) : G == 16 ? (uint32_t)((lane >> 2) & 1) : 0u;
     const uint32_t sbias_w = sbase + C::OFF_BIAS + warp * G * 4;
     for (int T = set; T < total; T += C::NSET) {
       const int gl = T >> tsh;
@@ -272,46 +280,46 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
       if (lane == 0) bulk_wait_read<0>();                      // this warp's previous TMA store has read the staging rows
       if (p.bias) {
 #pragma unroll
-        for (int i = 0; i < G / 32; ++i) {
+        for (int i = 0; i < NCH; ++i) {
           const int l = i * 32 + lane;
-          sts32(sbias_w + l * 4, __float_as_uint(l < nl ? __ldg(p.bias + g * G + l) : 0.f));
+          if (G >= 32 || l < G) sts32(sbias_w + l * 4, __float_as_uint(l < nl ? __ldg(p.bias + g * G + l) : 0.f));
         }
       }
       __syncwarp();
       // positives of this row inside the group: walk the CSR cursor (ascending groups, fixed row)
       const int64_t glo64 = p.label_offset + g * G;
       const int glo = (int)min(glo64, (int64_t)0x7fffffff), ghi = (int)min(glo64 + nl, (int64_t)0x7fffffff);
-      uint32_t ym[G / 32];
+      uint32_t ym[NCH];
 #pragma unroll
-      for (int i = 0; i < G / 32; ++i) ym[i] = 0;
+      for (int i = 0; i < NCH; ++i) ym[i] = 0;
       while (nxt < ghi) {
         if (nxt >= glo) {
           const int o = nxt - glo;
 #pragma unroll
-          for (int i = 0; i < G / 32; ++i) if ((o >> 5) == i) ym[i] |= 1u << (o & 31);
+          for (int i = 0; i < NCH; ++i) if ((o >> 5) == i) ym[i] |= 1u << (o & 31);
         }
         ++pc;
         nxt = pc < pe ? __ldg(p.col + pc) : 0x7fffffff;
       }
       uint32_t anyy = 0;
 #pragma unroll
-      for (int i = 0; i < G / 32; ++i) anyy |= ym[i];
+      for (int i = 0; i < NCH; ++i) anyy |= ym[i];
       const bool slow = __any_sync(0xffffffffu, anyy != 0) || nl < G || p.logits != nullptr;
 
       mbar_wait(&t_full[slot], (T / C::NSLOT) & 1);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * G;
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + slot * C::GP;
       float R[4] = {0.f, 0.f, 0.f, 0.f}, P[4] = {1.f, 1.f, 1.f, 1.f};
       uint32_t v[32];                 // one chunk at a time: 16 epilogue warps hide the TMEM latency, registers are short
       // two chunks are unrolled; four copies of the epilogue code (G = 128) overflow the instruction cache (see tc_head.cu)
 #pragma unroll(G >= 128 ? 1 : 2)
-      for (int sc = 0; sc < G / 32; ++sc) {
+      for (int sc = 0; sc < NCH; ++sc) {
         uint32_t ymsc = ym[0];
 #pragma unroll
-        for (int i = 1; i < G / 32; ++i) if (sc == i) ymsc = ym[i];
-        tmem_ld32(taddr + sc * 32, v);
+        for (int i = 1; i < NCH; ++i) if (sc == i) ymsc = ym[i];
+        tmem_ld_first<CW>(taddr + sc * 32, v);
         tmem_ld_wait();
-        if (sc + 1 == G / 32) {
+        if (sc + 1 == NCH) {
           // all of this warp's TMEM reads are done: hand the accumulator slot back to the MMA issuer
           tc_fence_before();
           __syncwarp();
@@ -325,7 +333,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
           // A thread inserts ~KL ln(n / KL) times over the n labels it sees, so most runs of 8 logits hold nothing above its
           // KL-th best: four 3-input maxima per run find that out, and only the runs that do are looked at one by one.
 #pragma unroll
-          for (int r8 = 0; r8 < 4; ++r8) {
+          for (int r8 = 0; r8 < CW / 8; ++r8) {
             float z[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -361,7 +369,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
           }
         } else if constexpr (TOPK < 0) {    // logits-only forward: z (+ bias) rounded to bf16, padding labels (>= L) written as zero
 #pragma unroll
-          for (int j = 0; j < 32; j += 2) {
+          for (int j = 0; j < CW; j += 2) {
             float z0 = __uint_as_float(v[j]), z1 = __uint_as_float(v[j + 1]);
             if (p.bias) {
               float b0, b1;
@@ -371,11 +379,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
             out[j >> 1] = pack_bf16x2(j < nvalid ? z0 : 0.f, j + 1 < nvalid ? z1 : 0.f);
           }
         } else if (slow) {
-          if (p.bias) epi32<true, true>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
-          else epi32<true, false>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
+          if (p.bias) epi32<true, true, CW>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
+          else epi32<true, false, CW>(v, sb, ymsc, nvalid, p.s, hs, R, P, out, zout);
         } else {
-          if (p.bias) epi32<false, true>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
-          else epi32<false, false>(v, sb, 0u, 32, p.s, hs, R, P, out, nullptr);
+          if (p.bias) epi32<false, true, CW>(v, sb, 0u, CW, p.s, hs, R, P, out, nullptr);
+          else epi32<false, false, CW>(v, sb, 0u, CW, p.s, hs, R, P, out, nullptr);
         }
         if (sc & 1) {   // 64 factors in [1/2,1) at most per product: fold into the loss, restart the chains
           loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
@@ -388,11 +396,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
             __syncwarp();
           }
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
+          for (int i = 0; i < CW / 8; ++i) {
             const uint32_t ch = (uint32_t)((G >= 64 ? (sc & 1) * 4 : 0) + i) ^ swz;
             sts128(stage_row + ch * 16, out[4 * i], out[4 * i + 1], out[4 * i + 2], out[4 * i + 3]);
           }
-          if (sc == G / 32 - 1 || (G > 64 && sc == 1)) {
+          if (sc == NCH - 1 || (G > 64 && sc == 1)) {
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) {
@@ -402,7 +410,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
           }
         }
       }
-      if ((G / 32) & 1)
+      if (NCH & 1)
         loss_local += (R[0] + R[1]) + (R[2] + R[3]) - 0.69314718056f * __log2f((P[0] * P[1]) * (P[2] * P[3]));
     }
     if (lane == 0) bulk_wait<0>();
@@ -435,7 +443,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
 // ---------------------------------------------------------------------------------------------
 bool tc_tail_supported(const haste_config_t& cfg, int) {
   if (cfg.dtype != HASTE_BF16) return false;
-  if (!(cfg.G == 32 || cfg.G == 64 || cfg.G == 128)) return false;
+  if (!(cfg.G == 8 || cfg.G == 16 || cfg.G == 32 || cfg.G == 64 || cfg.G == 128)) return false;
   if (!(cfg.K == 64 || cfg.K == 128)) return false;
   if (cfg.L < 1 || cfg.B_max > 128 * 2 * 128) return false;
   return true;
@@ -475,7 +483,7 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
     const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
     const uint32_t box[3] = {(uint32_t)std::min(G, 64), 32, 1};   // one epilogue warp's 32 rows
-    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : G * 2);   // 16-byte rows (G = 8): no swizzle
     if (rc) return rc;
   } else {
     tmY = tmW;
@@ -515,6 +523,7 @@ int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const i
 #define HASTE_FWD(G_, K_) \
   if (sh.G == G_ && sh.K == K_) return launch_fwd<G_, K_>(s, sh, Xt, idx, W, bias, rowptr, col, loss_partials, loss, dY, logits_out, z_mode, topk_val, topk_idx, geom, st)
   HASTE_FWD(64, 128); HASTE_FWD(64, 64); HASTE_FWD(32, 64); HASTE_FWD(32, 128); HASTE_FWD(128, 64); HASTE_FWD(128, 128);
+  HASTE_FWD(16, 64); HASTE_FWD(16, 128); HASTE_FWD(8, 64); HASTE_FWD(8, 128);
 #undef HASTE_FWD
   set_error("tcgen05 forward: unsupported (G, K)");
   return HASTE_ERR_UNSUPPORTED;

@@ -73,6 +73,10 @@ SMALL = [
     (256, 256, 128 * 3 + 5, 128, 128, "bf16", True, True),
     (512, 768, 64 * 40 + 11, 64, 128, "bf16", True, True),   # config-3 tile shape, several tiles, ragged tail
     (100, 200, 64 * 3 + 1, 64, 24, "bf16", False, True),     # shape outside the tensor-core family
+    (130, 256, 16 * 19 + 5, 16, 64, "bf16", True, True),     # narrow groups on the tensor cores: G = 16 ...
+    (300, 384, 16 * 40 + 9, 16, 128, "bf16", True, False),
+    (200, 256, 8 * 37 + 3, 8, 64, "bf16", True, True),       # ... and G = 8 (MMA N = 16, half of it unused)
+    (129, 512, 8 * 50 + 1, 8, 128, "bf16", False, True),     # unsorted idx rows: dX takes the L2 path for every slot
 ]
 
 
@@ -114,7 +118,8 @@ def test_stage_isolated_backward(oracle, H, force_simt):
 
 
 @pytest.mark.parametrize("force_simt", [False, True])
-@pytest.mark.parametrize("shape", [(64, 96, 64 * 3 + 5, 64, 64), (40, 64, 77, 8, 16), (128, 256, 32 * 5 + 3, 32, 64)])
+@pytest.mark.parametrize("shape", [(64, 96, 64 * 3 + 5, 64, 64), (40, 64, 77, 8, 16), (128, 256, 32 * 5 + 3, 32, 64),
+                                   (200, 128, 16 * 9 + 3, 16, 64), (130, 256, 8 * 21 + 5, 8, 128)])
 def test_integer_exactness(oracle, H, shape, force_simt):
     """P7: small-integer X, W, dY (exact in bf16, every partial sum < 2^24): logits, dW and dX must
     equal the oracle EXACTLY whatever the accumulation or atomic order -- gather/scatter addressing
@@ -273,7 +278,8 @@ def test_trained_regime_confident_negatives(oracle, H, force_simt):
     _check_backward(oracle, bout, bref, 5e-3, G)
 
 
-@pytest.mark.parametrize("shape", [(300, 768, 64 * 23 + 11, 64, 128), (130, 256, 32 * 9 + 5, 32, 64), (64, 512, 128 * 5 + 3, 128, 128)])
+@pytest.mark.parametrize("shape", [(300, 768, 64 * 23 + 11, 64, 128), (130, 256, 32 * 9 + 5, 32, 64), (64, 512, 128 * 5 + 3, 128, 128),
+                                   (200, 256, 16 * 30 + 7, 16, 64), (130, 384, 8 * 50 + 3, 8, 128)])
 @pytest.mark.parametrize("with_bias", [False, True])
 def test_forward_logits_only(oracle, H, shape, with_bias):
     """haste_forward_logits: z = bias + sum_j W[l,j] X[i, idx[l/G, j]] rounded once to bf16, in the library

@@ -32,7 +32,8 @@ def _check_topk(z_ref, got_val, got_idx, k, label_offset=0, tol=2e-5):
 
 
 @pytest.mark.parametrize("shape", [(300, 768, 64 * 23 + 11, 64, 128), (130, 256, 32 * 40 + 5, 32, 64), (64, 512, 128 * 5 + 3, 128, 128),
-                                   (257, 768, 64 * 300 + 1, 64, 64), (33, 256, 5, 64, 64)])
+                                   (257, 768, 64 * 300 + 1, 64, 64), (33, 256, 5, 64, 64),
+                                   (200, 256, 16 * 90 + 7, 16, 64), (130, 384, 8 * 150 + 3, 8, 128)])
 @pytest.mark.parametrize("k", [1, 5, 8])
 def test_forward_topk_small(oracle, shape, k):
     from gpu_util import TailRun
