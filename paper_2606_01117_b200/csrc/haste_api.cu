@@ -200,7 +200,7 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
   if (cfg->flags & HASTE_DETERMINISTIC) {
     // atomic-free dX: only the accumulating tcgen05 kernel has such a variant (private partial tiles + ordered reduction)
     if (h->family != 1) {
-      set_error("haste_create: HASTE_DETERMINISTIC needs a shape of the tcgen05 family (bf16, G in {32,64,128}, K in {64,128})");
+      set_error("haste_create: HASTE_DETERMINISTIC needs a shape of the tcgen05 family (bf16, G in {8,16,32,64,128}, K in {64,128})");
       haste_destroy(h);
       return HASTE_ERR_UNSUPPORTED;
     }
@@ -491,7 +491,7 @@ int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* id
     return HASTE_ERR_INVALID_ARG;
   }
   if (h->family != 1 || h->dx_part) {
-    set_error("haste_backward_sgd: needs the tcgen05 kernel family (bf16, G in {32,64,128}, K in {64,128}) without HASTE_DETERMINISTIC");
+    set_error("haste_backward_sgd: needs the tcgen05 kernel family (bf16, G in {8,16,32,64,128}, K in {64,128}) without HASTE_DETERMINISTIC");
     return HASTE_ERR_UNSUPPORTED;
   }
   DeviceGuard guard(h->device);
@@ -512,6 +512,7 @@ int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* id
   if (dX) {        // the input gradient first: it needs W as it was in the forward, the update below overwrites it
     pf.begin(HASTE_KERNEL_DX, st);
     rc = tc_tail_dx(h->tc, sh, idx, W, dY, h->dXt, nullptr, st, &n);
+    if (rc == HASTE_ERR_UNSUPPORTED) set_error("haste_backward_sgd: no tcgen05 dX kernel for G = %d, K = %d, B = %d", sh.G, sh.K, B);
     if (rc) return rc;
     h->last_launches += n;
     pf.end(HASTE_KERNEL_DX, st);

@@ -21,7 +21,7 @@ int tc_tail_num_sms(const TcTailState* s) { return s->num_sms; }
 int tc_tail_dx(TcTailState* s, const TailShape& sh, const int32_t* idx, const void* W, const void* dY, float* dXt,
                float* dx_part, cudaStream_t st, int* n_launches) {
   *n_launches = 1;
-  if (!((sh.G == 32 || sh.G == 64 || sh.G == 128) && (sh.K == 64 || sh.K == 128))) return HASTE_ERR_UNSUPPORTED;
+  if (!((sh.G == 8 || sh.G == 16 || sh.G == 32 || sh.G == 64 || sh.G == 128) && (sh.K == 64 || sh.K == 128))) return HASTE_ERR_UNSUPPORTED;
   return tc_tail_dx_acc(s, sh, idx, W, dY, dXt, dx_part, st);
 }
 

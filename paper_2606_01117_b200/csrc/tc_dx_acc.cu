@@ -46,9 +46,14 @@ struct DxAccParams {
 template <int G, int K, int NST_> struct DxAccCfg {
   static constexpr int NSET = 4;                              // epilogue sets: 0 = TA, 1 = SB, 2 = TC, 3 = SD
   static constexpr int NLIST = NSET + 1;                      // + the L list
-  static constexpr int Y_BYTES = G * 256;                     // [G/64 k-blocks][128 batch rows][128 B]; G = 32: [128 rows][64 B]
-  static constexpr int W_BYTES = G * K * 2;                   // [K/64 slot atoms][G label rows][128 B]
+  // narrow groups: the contraction (over the group's labels) is GP = 16 long, the shortest bf16 MMA.  G = 8: the dY box is
+  // 16 labels wide over rows that have 8, so labels 8-15 arrive as zeros, and label rows 8-15 of the W image are zeroed
+  // once and never loaded.
+  static constexpr int GP = G < 16 ? 16 : G;
+  static constexpr int Y_BYTES = GP * 256;                    // [G/64 k-blocks][128 batch rows][128 B]; G = 32: [128 rows][64 B]; G <= 16: [128 rows][32 B]
+  static constexpr int W_BYTES = GP * K * 2;                  // [K/64 slot atoms][GP label rows][128 B]
   static constexpr int STAGE = Y_BYTES + W_BYTES;
+  static constexpr int TX_BYTES = Y_BYTES + G * K * 2;        // what the TMA boxes of one group bring
   static constexpr int NST = NST_;                            // operand stages (dY tile + W_g) in flight
   static constexpr int LIST_LEN = K + 16;                     // entries per list (padding for the last chunk)
   static constexpr int RING_META = 48;                        // lo[5] at 0, n[5] at 20
@@ -202,6 +207,13 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     fence_barrier_init();
   }
   if (warp == 4 * C::NSET + 1 && lane == 0) { tma_prefetch_desc(&tmY); tma_prefetch_desc(&tmW); }
+  if constexpr (G < 16) {               // label rows 8-15 of every W image: zero (see DxAccCfg)
+    for (int e = threadIdx.x; e < C::NST * (K / 64) * 64; e += blockDim.x) {
+      const int st = e / ((K / 64) * 64), a = (e / 64) % (K / 64), c = e % 64;
+      sts128(sbase + st * C::STAGE + C::Y_BYTES + a * (C::GP * 128) + 1024 + c * 16, 0u, 0u, 0u, 0u);
+    }
+    fence_proxy_async_smem();
+  }
   if (warp == 4 * C::NSET) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
@@ -215,12 +227,12 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         const int64_t g = stripe + (int64_t)i * p.S;
         const int st = i % C::NST;
         mbar_wait(&empty[st], ((i / C::NST) & 1) ^ 1);
-        mbar_arrive_expect_tx(&full[st], C::STAGE);
+        mbar_arrive_expect_tx(&full[st], C::TX_BYTES);
         uint8_t* s0 = smem + st * C::STAGE;
 #pragma unroll
         for (int kb = 0; kb < (G >= 64 ? G / 64 : 1); ++kb) tma_load_3d(s0 + kb * 16384, &tmY, &full[st], kb * 64, bt * 128, (int)g);
 #pragma unroll
-        for (int a = 0; a < K / 64; ++a) tma_load_2d(s0 + C::Y_BYTES + a * (G * 128), &tmW, &full[st], a * 64, (int)(g * G));
+        for (int a = 0; a < K / 64; ++a) tma_load_2d(s0 + C::Y_BYTES + a * (C::GP * 128), &tmW, &full[st], a * 64, (int)(g * G));
       }
     }
   } else if (warp == 4 * C::NSET) {
@@ -228,8 +240,9 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     // whole warp waits, one elected lane issues; descriptors are a per-stage base + compile-time offsets (see tc_tail.cu)
     constexpr uint32_t idesc = make_idesc_bf16(128, K, /*A (dY) K-major*/ 0, /*B (W) MN-major*/ 1);
     // A = the dY tile, K-major: 128-byte rows (64 labels per k-block) or, for G = 32, 64-byte rows with the 64-byte swizzle
-    const uint64_t adesc0 = G >= 64 ? make_sdesc_sw128(sbase, 16, 1024) : make_sdesc_sw64(sbase, 16, 512);
-    const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::Y_BYTES, G * 128, 1024);
+    // (G <= 16: 32-byte rows with the 32-byte swizzle)
+    const uint64_t adesc0 = G >= 64 ? make_sdesc_sw128(sbase, 16, 1024) : G == 32 ? make_sdesc_sw64(sbase, 16, 512) : make_sdesc_sw32(sbase, 16, 256);
+    const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::Y_BYTES, C::GP * 128, 1024);
     for (int i = 0; i < n_my; ++i) {
       const int st = i % C::NST, slot = i & 1;
       dxa_wait2(&full[st], (i / C::NST) & 1, &t_empty[slot], ((i >> 1) & 1) ^ 1);
@@ -238,7 +251,7 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         const uint64_t so = (uint64_t)((st * C::STAGE) >> 4);
         const uint32_t d = tmem_base + slot * K;
 #pragma unroll
-        for (int j = 0; j < G / 16; ++j)
+        for (int j = 0; j < C::GP / 16; ++j)
           umma_f16(d, adesc0 + so + (uint64_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4), bdesc0 + so + (uint64_t)((j * 2048) >> 4),
                    idesc, j ? 1u : 0u);
         umma_commit(&empty[st]);
@@ -451,8 +464,8 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   {
     const uint64_t dims[3] = {(uint64_t)G, (uint64_t)sh.B, (uint64_t)sh.NG};
     const uint64_t str[2] = {(uint64_t)G * 2, (uint64_t)sh.B * G * 2};
-    const uint32_t box[3] = {(uint32_t)std::min(G, 64), 128, 1};
-    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : 64);
+    const uint32_t box[3] = {(uint32_t)std::min(C::GP, 64), 128, 1};
+    int rc = encode_tmap(&tmY, 2, dY, 3, dims, str, box, G >= 64 ? 128 : G == 32 ? 64 : 32);
     if (rc) return rc;
   }
   {
@@ -490,6 +503,7 @@ int tc_tail_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx, cons
   if (sh.G == G_ && sh.K == K_) return launch_dx_acc<G_, K_, 2>(s, sh, idx, W, dY, dXt, part, st)
   HASTE_DXA(64, 128); HASTE_DXA(64, 64); HASTE_DXA(128, 64); HASTE_DXA(128, 128);
   HASTE_DXA(32, 64); HASTE_DXA(32, 128);
+  HASTE_DXA(16, 64); HASTE_DXA(16, 128); HASTE_DXA(8, 64); HASTE_DXA(8, 128);
 #undef HASTE_DXA
   return HASTE_ERR_UNSUPPORTED;
 }

@@ -12,7 +12,8 @@ from paper_2606_01117_b200 import synth
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("shape", [(300, 768, 64 * 700 + 3, 64, 128), (200, 1024, 64 * 300 + 9, 64, 64), (130, 768, 32 * 401, 32, 64)])
+@pytest.mark.parametrize("shape", [(300, 768, 64 * 700 + 3, 64, 128), (200, 1024, 64 * 300 + 9, 64, 64), (130, 768, 32 * 401, 32, 64),
+                                   (200, 768, 16 * 500 + 3, 16, 64), (130, 512, 8 * 700 + 1, 8, 128)])
 def test_tail_dx_deterministic(oracle, shape):
     from paper_2606_01117_b200 import haste
     from gpu_util import TailRun, dy_rounded

@@ -52,6 +52,10 @@ CASES = [
     (257, 768, 40, 64, 128, "strict"),    # every row strictly increasing (the fast path only)
     (200, 768, 21, 32, 64, "mixed"),      # config-2 tile shape: G = 32 (dY tile is a 64-byte-swizzle operand)
     (130, 768, 13, 32, 128, "mixed"),
+    (200, 768, 41, 16, 64, "mixed"),      # narrow groups: the dY tile is a 32-byte-swizzle operand, one MMA per group
+    (130, 1024, 37, 16, 128, "mixed"),
+    (300, 768, 53, 8, 64, "mixed"),       # G = 8: labels 8-15 of the operands are zero padding (TMA fill / zeroed W rows)
+    (129, 600, 29, 8, 128, "mixed"),
 ]
 
 

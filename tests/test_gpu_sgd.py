@@ -18,7 +18,8 @@ def _bf16_step(x):
 
 
 @pytest.mark.parametrize("shape", [(300, 768, 64 * 23 + 11, 64, 128), (130, 256, 32 * 40 + 5, 32, 64), (64, 512, 128 * 5 + 3, 128, 128),
-                                   (257, 768, 64 * 200 + 1, 64, 64), (200, 512, 128 * 9, 128, 64)])
+                                   (257, 768, 64 * 200 + 1, 64, 64), (200, 512, 128 * 9, 128, 64),
+                                   (130, 256, 32 * 21 + 5, 32, 128), (200, 256, 16 * 50 + 7, 16, 64), (130, 384, 8 * 90 + 3, 8, 128)])
 @pytest.mark.parametrize("with_bias", [False, True])
 def test_backward_sgd_two_steps(oracle, shape, with_bias):
     from gpu_util import TailRun, dy_rounded
