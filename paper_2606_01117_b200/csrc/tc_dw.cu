@@ -67,7 +67,9 @@ template <int G, int K, bool F32, bool SGD = false> struct DwCfg {
   static constexpr int EPI_BYTES = 4 * 4096;                // 4 warps x [32 rows][128 B]
   static constexpr int NST_RAW = (232448 - 1024 - EPI_BYTES - 1024) / STAGE;
   static constexpr int NST = NST_RAW > 8 ? 8 : NST_RAW;
-  static constexpr int LAG = 2;
+  // producer completion lag: LAG + 1 k-blocks of cp.async in flight per producer warp.  A narrow group's k-block is the same
+  // gather for a fraction of the labels, so there the gather's latency is what bounds the kernel: more in flight
+  static constexpr int LAG = (G <= 16 && NST >= 7) ? 4 : 2;
   static constexpr int TS = N <= 128 ? 128 : 256;           // TMEM columns per accumulator slot
   static constexpr int OFF_EPI = NST * STAGE;
   static constexpr int OFF_BAR = OFF_EPI + EPI_BYTES;
@@ -172,7 +174,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     for (int r = C::LAG - 1; r >= 0; --r) {
       const int T = it - 1 - r;
       if (T >= 0) {
-        if (r == 1) cp_async_wait<1>(); else cp_async_wait<0>();
+        if (r == 3) cp_async_wait<3>(); else if (r == 2) cp_async_wait<2>(); else if (r == 1) cp_async_wait<1>(); else cp_async_wait<0>();
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(&full[T % C::NST]);

@@ -84,7 +84,17 @@ struct FwdParams {
 
 template <int G, int K> struct FwdCfg {
   static constexpr int NSET = (G == 128 && K == 128) ? 2 : 4;   // epilogue sets (4 warps each); what shared memory allows
-  static constexpr int HS = 3;                                  // H stages
+  // Narrow groups (G <= 16): a tile is as many gathered bytes as a wide group's but a quarter (an eighth) of the work
+  // after it, and what bounds it is the hand-shaking itself: with the wide groups' six barriers per tile and no work at
+  // all in any role the kernel took as long as with all of it (config 5, B = 1024, G = 16: 0.79 vs 0.80 ms; a barrier
+  // wait costs the waiting warp 100-300 cycles even when it succeeds at once).  So NARROW runs ONE ring of R entries
+  // -- H stage, W stage and TMEM slot e = T mod R belong together -- with two barriers per entry:
+  //   ready[e]: the producer warp's gather has landed + the W box has landed + the four epilogue warps have drained
+  //             the slot (its previous use);   done[e]: the tile's MMAs have completed (one commit).
+  // The issuer waits once and commits once per tile; each producer warp takes every fourth tile whole, so its own chain
+  // (wait, issue, wait for the copies, fence, arrive) is a quarter as often on the critical path.
+  static constexpr bool NARROW = G <= 16;
+  static constexpr int HS = NARROW ? (K <= 64 ? 8 : 5) : 3;     // H stages (NARROW: the ring length R)
   static constexpr int LAG = 1;                                 // producer completion lag (< HS-1, or the MMAs serialise)
   // narrow groups (G = 16, 8): the MMA is N = GP = 16 wide (the smallest N of an M = 128 MMA); for G = 8 the upper 8 rows
   // of the W image are never written and the 8 accumulator columns they produce are never read
@@ -94,9 +104,9 @@ template <int G, int K> struct FwdCfg {
   static constexpr int H_BYTES = K * 256;                       // [2 m-blocks][K rows][128 B]
   static constexpr int W_BYTES = GP * K * 2;                    // [K/64 k-blocks][GP rows][128 B]
   static constexpr int W_TX = G * K * 2;                        // bytes the TMA box of a group brings
-  static constexpr int WS = W_BYTES <= 16384 ? 3 : 2;           // W stages
+  static constexpr int WS = NARROW ? HS : W_BYTES <= 16384 ? 3 : 2;   // W stages
   static constexpr int ST_BYTES = 128 * (G < 64 ? G : 64) * 2;  // one dY staging tile (<= 64 labels wide) per epilogue set
-  static constexpr int NSLOT = (512 / GP) >= 8 ? 8 : (512 / GP);  // TMEM accumulator ring (GP columns each)
+  static constexpr int NSLOT = NARROW ? HS : (512 / GP) >= 8 ? 8 : (512 / GP);  // TMEM accumulator ring (GP columns each)
   static constexpr int OFF_H = 0;
   static constexpr int OFF_W = OFF_H + HS * H_BYTES;
   static constexpr int OFF_ST = OFF_W + WS * W_BYTES;
@@ -120,10 +130,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
   uint64_t* h_full = bars;                       // [HS]  count 4 (producer warps)
   uint64_t* h_empty = bars + C::HS;              // [HS]  count 1 (umma commit)
-  uint64_t* w_full = bars + 2 * C::HS;           // [WS]  count 1 + tx
-  uint64_t* w_empty = w_full + C::WS;            // [WS]  count 1 (umma commit)
-  uint64_t* t_full = w_empty + C::WS;            // [NSLOT] count 1 (umma commit)
-  uint64_t* t_empty = t_full + C::NSLOT;         // [NSLOT] count 4 (epilogue warps of one set)
+  // NARROW: h_full = w_full = t_empty = ready[R] (count 6 + tx), h_empty = w_empty = t_full = done[R] (count 1)
+  uint64_t* w_full = C::NARROW ? h_full : bars + 2 * C::HS;           // [WS]  count 1 + tx
+  uint64_t* w_empty = C::NARROW ? h_empty : w_full + C::WS;           // [WS]  count 1 (umma commit)
+  uint64_t* t_full = C::NARROW ? h_empty : w_empty + C::WS;           // [NSLOT] count 1 (umma commit)
+  uint64_t* t_empty = C::NARROW ? h_full : t_full + C::NSLOT;         // [NSLOT] count 4 (epilogue warps of one set)
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_MISC);
   float* loss_red = reinterpret_cast<float*>(smem + C::OFF_MISC + 16);   // [4 * NSET]
 
@@ -135,9 +146,16 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   const int total = ngl << tsh;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < C::HS; ++i) { mbar_init(&h_full[i], 4); mbar_init(&h_empty[i], 1); }
-    for (int i = 0; i < C::WS; ++i) { mbar_init(&w_full[i], 1); mbar_init(&w_empty[i], 1); }
-    for (int i = 0; i < C::NSLOT; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
+    if constexpr (C::NARROW) {
+      for (int i = 0; i < C::HS; ++i) {
+        mbar_init(&h_full[i], 6); mbar_init(&h_empty[i], 1);
+        for (int a = 0; a < 4; ++a) mbar_arrive(&h_full[i]);       // first round: no earlier use of the slot to drain
+      }
+    } else {
+      for (int i = 0; i < C::HS; ++i) { mbar_init(&h_full[i], 4); mbar_init(&h_empty[i], 1); }
+      for (int i = 0; i < C::WS; ++i) { mbar_init(&w_full[i], 1); mbar_init(&w_empty[i], 1); }
+      for (int i = 0; i < C::NSLOT; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
+    }
     fence_barrier_init();
   }
   constexpr int EW = 4 * C::NSET;                                          // epilogue warps
@@ -151,6 +169,52 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   if (warp >= EW && warp < EW + 4) {
     // ===================== gather producers =====================
     const int pw = warp - EW;
+    if constexpr (C::NARROW) {
+      // warp pw gathers tiles T = pw, pw + 4, ... whole: all K rows, two rows per instruction, two tiles in flight
+      const int sub = lane >> 4, c = lane & 15;
+      const uint32_t dst_lane = (uint32_t)((c >> 3) * (K * 128) + (((c & 7)) << 4));
+      constexpr int NI = K / 32;                     // lane holds slots lane + 32 t of the tile's idx row
+      int idx_cur[NI], idx_nxt[NI];
+      auto load_idx = [&](int T, int (&o)[NI]) {
+        const int64_t g = stripe + (int64_t)(T >> tsh) * p.S;
+#pragma unroll
+        for (int t = 0; t < NI; ++t) o[t] = T < total ? __ldg(p.idx + g * K + lane + 32 * t) : 0;
+      };
+      load_idx(pw, idx_nxt);
+      int prev_hs = -1;
+      for (int T = pw; T < total; T += 4) {
+        const int which = T & tsh;
+#pragma unroll
+        for (int t = 0; t < NI; ++t) idx_cur[t] = idx_nxt[t];
+        load_idx(T + 4, idx_nxt);
+        const int hs = T % C::HS;
+        mbar_wait(&h_empty[hs], ((T / C::HS) & 1) ^ 1);
+        const int b0 = (2 * pr + which) * 128;
+        const uint32_t dst0 = sbase + C::OFF_H + hs * C::H_BYTES + dst_lane;
+        const bf16* src0 = p.Xt + b0 + c * 8;
+#pragma unroll
+        for (int i = 0; i < K / 2; ++i) {
+          const int k = 2 * i + sub;
+          const int f = __shfl_sync(0xffffffffu, idx_cur[(2 * i) >> 5], k & 31);
+          const uint32_t dst = (dst0 + k * 128) ^ ((uint32_t)(k & 7) << 4);
+          cp_async16(dst, src0 + (size_t)f * p.Bpad);
+        }
+        cp_async_commit();
+        if (prev_hs >= 0) {
+          cp_async_wait<1>();
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&h_full[prev_hs]);
+        }
+        prev_hs = hs;
+      }
+      if (prev_hs >= 0) {
+        cp_async_wait<0>();
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&h_full[prev_hs]);
+      }
+    } else {
     constexpr int RPW = K / 4;                       // rows (slots) per producer warp
     const int sub = lane >> 4, c = lane & 15;        // two rows per instruction, 16 chunks of 16 B per row
     const uint32_t dst_lane = (uint32_t)((c >> 3) * (K * 128) + (((c & 7)) << 4));
@@ -195,11 +259,12 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     for (int r = C::LAG - 1; r >= 0; --r) {
       const int T = total - 1 - r;
       if (T >= 0) {
-        if (r == 1) cp_async_wait<1>(); else cp_async_wait<0>();
+        if (r == 2) cp_async_wait<2>(); else if (r == 1) cp_async_wait<1>(); else cp_async_wait<0>();
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(&h_full[T % C::HS]);
       }
+    }
     }
   } else if (warp == EW + 4) {
     // ===================== MMA issuer =====================
@@ -211,10 +276,14 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     const uint64_t bdesc0 = make_sdesc_sw128(sbase + C::OFF_W, 16, 1024);
     for (int T = 0; T < total; ++T) {
       const int gl = T >> tsh, which = T & tsh;
-      const int ws = gl % C::WS, hs = T % C::HS, slot = T % C::NSLOT;
-      if (which == 0) mbar_wait(&w_full[ws], (gl / C::WS) & 1);
-      mbar_wait(&h_full[hs], (T / C::HS) & 1);
-      mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
+      const int ws = C::NARROW ? T % C::HS : gl % C::WS, hs = T % C::HS, slot = T % C::NSLOT;
+      if constexpr (C::NARROW) {
+        mbar_wait(&h_full[hs], (T / C::HS) & 1);                // ready: gather + W landed, slot drained
+      } else {
+        if (which == 0) mbar_wait(&w_full[ws], (gl / C::WS) & 1);
+        mbar_wait(&h_full[hs], (T / C::HS) & 1);
+        mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
+      }
       tc_fence_after();
       if (elect_one()) {
         const uint64_t ad0 = adesc0 + (uint64_t)((hs * C::H_BYTES) >> 4);       // the address field never carries out
@@ -224,15 +293,27 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
         for (int j = 0; j < K / 16; ++j)
           umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * (C::GP * 128) + (j & 3) * 32) >> 4), idesc,
                    j > 0 ? 1u : 0u);
-        umma_commit(&h_empty[hs]);
-        umma_commit(&t_full[slot]);
-        if (which == tsh) umma_commit(&w_empty[ws]);
+        umma_commit(&h_empty[hs]);                              // NARROW: done[e], the only commit
+        if constexpr (!C::NARROW) {
+          umma_commit(&t_full[slot]);
+          if (which == tsh) umma_commit(&w_empty[ws]);
+        }
       }
       __syncwarp();
     }
   } else if (warp == EW + 5) {
     // ===================== W loader =====================
-    if (lane == 0) {
+    if (C::NARROW && lane == 0) {                               // one (small) W box per tile, into the tile's ring entry
+      for (int T = 0; T < total; ++T) {
+        const int e = T % C::HS;
+        const int64_t g = stripe + (int64_t)(T >> tsh) * p.S;
+        mbar_wait(&h_empty[e], ((T / C::HS) & 1) ^ 1);
+        mbar_arrive_expect_tx(&h_full[e], C::W_TX);
+#pragma unroll
+        for (int kb = 0; kb < K / 64; ++kb)
+          tma_load_2d(smem + C::OFF_W + e * C::W_BYTES + kb * (C::GP * 128), &tmW, &h_full[e], kb * 64, (int)(g * G));
+      }
+    } else if (lane == 0) {
       for (int gl = 0; gl < ngl; ++gl) {
         const int ws = gl % C::WS;
         const int64_t g = stripe + (int64_t)gl * p.S;
@@ -272,6 +353,16 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
     const uint32_t stage_row = stage_w + lane * ROWB;
     const uint32_t swz = G >= 64 ? (uint32_t)(lane & 7) : G == 32 ? (uint32_t)((lane >> 1) & 3) : G == 16 ? (uint32_t)((lane >> 2) & 1) : 0u;
     const uint32_t sbias_w = sbase + C::OFF_BIAS + warp * G * 4;
+    // the group's bias values, fetched one of this warp's tiles ahead (a global load at the head of a tile's chain would
+    // be ~700 cycles nothing else in the warp hides)
+    auto bias_of = [&](int T, int i) -> float {
+      const int64_t gg = stripe + (int64_t)(T >> tsh) * p.S;
+      const int l = i * 32 + lane;
+      return (T < total && (G >= 32 || l < G) && gg * G + l < p.L) ? __ldg(p.bias + gg * G + l) : 0.f;
+    };
+    float bnext[NCH];
+#pragma unroll
+    for (int i = 0; i < NCH; ++i) bnext[i] = p.bias ? bias_of(set, i) : 0.f;
     for (int T = set; T < total; T += C::NSET) {
       const int gl = T >> tsh;
       const int64_t g = stripe + (int64_t)gl * p.S;
@@ -282,7 +373,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
           const int l = i * 32 + lane;
-          if (G >= 32 || l < G) sts32(sbias_w + l * 4, __float_as_uint(l < nl ? __ldg(p.bias + g * G + l) : 0.f));
+          if (G >= 32 || l < G) sts32(sbias_w + l * 4, __float_as_uint(bnext[i]));
+          bnext[i] = bias_of(T + C::NSET, i);
         }
       }
       __syncwarp();
