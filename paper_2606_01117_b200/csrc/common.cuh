@@ -30,6 +30,28 @@ void set_error(const char* fmt, ...);
     }                                                                                         \
   } while (0)
 
+// ---- programmatic dependent launch (PDL) ----
+// Every kernel of a training step is launched with the programmatic-stream-serialization attribute and runs
+//     <prologue that touches no global memory>;  pdl_wait();  pdl_trigger();  <the kernel>
+// pdl_wait returns once the preceding kernel of the stream has completed and its writes are visible; pdl_trigger then lets
+// the NEXT kernel's CTAs be placed on SMs as this kernel's CTAs leave them, where they run their own prologue (barrier
+// init, TMEM allocation, descriptor prefetch) and block in their pdl_wait.  Launch latency and prologue thus overlap the
+// tail of the kernel before; the data dependence is unchanged (nothing is read or written before pdl_wait, and every kernel
+// launched this way waits, so completion is transitive along the stream).  After anything that is not a kernel launched
+// this way (a memset, an event) the attribute has no effect.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 static inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 static inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
 

@@ -88,6 +88,7 @@ struct haste_layer {
   int Bpad;         // row pitch of Xt / dXt
   void* Xt;         // [d][Bpad] dtype
   float* dXt;       // [d][Bpad] fp32
+  bool dxt_clean;   // dXt is all zero (the transpose-out kernel zeroes what it reads; false after a pass that ended early)
   float* dx_part;   // HASTE_DETERMINISTIC: [num_sms][d][128] fp32 private partial tiles of the dX kernel, else null
   double* loss_acc; // device scalar
   float* partials;  // [n_partials] per-CTA loss partials (tcgen05 family)
@@ -185,6 +186,8 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
   if (e == cudaSuccess) e = cudaMalloc(&h->partials, h->n_partials * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&h->flag, sizeof(int));
   if (e == cudaSuccess) e = cudaMemset(h->Xt, 0, xt_bytes);
+  if (e == cudaSuccess) e = cudaMemset(h->dXt, 0, dxt_bytes);
+  h->dxt_clean = (e == cudaSuccess);
   if (e == cudaSuccess) e = cudaMemset(h->partials, 0, h->n_partials * sizeof(float));
   if (e != cudaSuccess) {
     set_error("haste_create: workspace allocation failed: %s", cudaGetErrorString(e));
@@ -429,7 +432,10 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
     if (rc) return rc;
     h->last_launches++;
   }
-  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+  if (dX) {      // zero already unless an earlier pass ended between its dX kernel and the transpose-out (no memset between kernels: PDL)
+    if (!h->dxt_clean) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+    h->dxt_clean = false;
+  }
   pf.end(HASTE_KERNEL_PREP_BWD, st);
   if (dW || dbias) {
     pf.begin(HASTE_KERNEL_DW, st);
@@ -473,6 +479,7 @@ int haste_backward(haste_layer_t* h, int B, const void* X, const int32_t* idx, c
     pf.begin(HASTE_KERNEL_POST_BWD, st);
     rc = launch_untranspose_f32(h->dXt, dX, B, sh.d, h->Bpad, accumulate_dX, st);
     if (rc) return rc;
+    h->dxt_clean = true;
     h->last_launches++;
     pf.end(HASTE_KERNEL_POST_BWD, st);
   }
@@ -506,7 +513,10 @@ int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* id
     if (rc) return rc;
     h->last_launches++;
   }
-  if (dX) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+  if (dX) {      // zero already unless an earlier pass ended between its dX kernel and the transpose-out (no memset between kernels: PDL)
+    if (!h->dxt_clean) HASTE_CUDA_TRY(cudaMemsetAsync(h->dXt, 0, (size_t)sh.d * h->Bpad * 4, st));
+    h->dxt_clean = false;
+  }
   pf.end(HASTE_KERNEL_PREP_BWD, st);
   int n = 0;
   if (dX) {        // the input gradient first: it needs W as it was in the forward, the update below overwrites it
@@ -519,6 +529,7 @@ int haste_backward_sgd(haste_layer_t* h, int B, const void* X, const int32_t* id
     pf.begin(HASTE_KERNEL_POST_BWD, st);
     rc = launch_untranspose_f32(h->dXt, dX, B, sh.d, h->Bpad, accumulate_dX, st);
     if (rc) return rc;
+    h->dxt_clean = true;
     h->last_launches++;
     pf.end(HASTE_KERNEL_POST_BWD, st);
   }

@@ -9,7 +9,7 @@ namespace haste {
 // Xt[f][b] = X[b][f] for b < B, 0 for B <= b < Bzero (Bzero <= Bpad, the row pitch).
 int launch_transpose_pad(haste_dtype_t dt, const void* X, void* Xt, int B, int d, int Bpad, int Bzero, cudaStream_t st);
 // dX[b][f] (=|+=) dXt[f][b]
-int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st);
+int launch_untranspose_f32(float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st);
 // fused top-k: merge the forward kernel's per-thread candidates into the k best (value, global label id) per batch row
 int launch_topk_merge(const float* cand_val, const int* cand_idx, int NP, int S, int NSET, int NT, int B, int k,
                       int64_t label_offset, float* out_val, int64_t* out_idx, cudaStream_t st);

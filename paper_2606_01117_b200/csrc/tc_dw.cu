@@ -125,6 +125,8 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_wait();       // nothing above touches global memory (common.cuh, PDL)
+  pdl_trigger();
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp >= 4 && warp < 8) {
@@ -416,8 +418,7 @@ static int launch_dw(TcTailState* s, const TailShape& sh, const void* Xt, const 
   p.B = sh.B; p.Bpad = sh.Bpad; p.NKB = ceil_div(sh.B, 128); p.L = sh.L; p.NG = sh.NG;
   const int grid = (int)std::min<int64_t>(C::PAIR ? (sh.NG + 1) / 2 : sh.NG, s->num_sms);
   HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dw_kernel<G, K, F32, SGD>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-  tc_dw_kernel<G, K, F32, SGD><<<grid, 320, C::SMEM, st>>>(tmY, tmO, p);
-  HASTE_LAUNCH_CHECK();
+  HASTE_CUDA_TRY(launch_pdl(tc_dw_kernel<G, K, F32, SGD>, dim3(grid), dim3(320), C::SMEM, st, tmY, tmO, p));
   return HASTE_OK;
 }
 

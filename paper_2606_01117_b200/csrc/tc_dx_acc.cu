@@ -218,6 +218,8 @@ tc_dx_acc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_wait();       // nothing above touches global memory (common.cuh, PDL)
+  pdl_trigger();
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == 4 * C::NSET + 1) {
@@ -487,10 +489,10 @@ static int launch_dx_acc(TcTailState* s, const TailShape& sh, const int32_t* idx
   const int smem = C::OFF_ACC + (ns + 1) * 512 + 1024;
   if (part) {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K, NST, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    tc_dx_acc_kernel<G, K, NST, true><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_dx_acc_kernel<G, K, NST, true>, dim3(p.NT * p.S), dim3(C::THREADS), smem, st, tmY, tmW, p));
   } else {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_dx_acc_kernel<G, K, NST, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    tc_dx_acc_kernel<G, K, NST, false><<<p.NT * p.S, C::THREADS, smem, st>>>(tmY, tmW, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_dx_acc_kernel<G, K, NST, false>, dim3(p.NT * p.S), dim3(C::THREADS), smem, st, tmY, tmW, p));
   }
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;

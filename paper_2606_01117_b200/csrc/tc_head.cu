@@ -115,6 +115,8 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_wait();       // nothing above touches global memory (common.cuh, PDL)
+  pdl_trigger();
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == 5) {
@@ -401,6 +403,8 @@ tc_head_fwd256_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_cons
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_wait();       // nothing above touches global memory (common.cuh, PDL)
+  pdl_trigger();
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == C::NEW + 1) {
@@ -604,7 +608,7 @@ static int launch_head(TcHeadState* s, const CUtensorMap& tmA, const CUtensorMap
   const int n_items = p.MT * p.NTL * p.NSLAB;
   const int grid = std::min(n_items, s->num_sms);
   HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_head_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-  tc_head_kernel<MODE><<<grid, 192, C::SMEM, st>>>(tmA, tmB, tmO, p);
+  HASTE_CUDA_TRY(launch_pdl(tc_head_kernel<MODE>, dim3(grid), dim3(192), C::SMEM, st, tmA, tmB, tmO, p));
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;
 }
@@ -633,7 +637,7 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
     const int grid = std::min(p.MT * p.NTL, s->num_sms);
     static_assert(Fwd256Cfg::SMEM <= 232448, "shared memory budget");
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_head_fwd256_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Fwd256Cfg::SMEM));
-    tc_head_fwd256_kernel<<<grid, Fwd256Cfg::THREADS, Fwd256Cfg::SMEM, st>>>(tmA, tmB, tmO, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_head_fwd256_kernel, dim3(grid), dim3(Fwd256Cfg::THREADS), Fwd256Cfg::SMEM, st, tmA, tmB, tmO, p));
     HASTE_LAUNCH_CHECK();
     return HASTE_OK;
   }

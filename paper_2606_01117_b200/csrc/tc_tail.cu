@@ -164,6 +164,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ C
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_wait();       // nothing above touches global memory (common.cuh, PDL)
+  pdl_trigger();
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp >= EW && warp < EW + 4) {
@@ -593,16 +595,16 @@ static int launch_fwd(TcTailState* s, const TailShape& sh, const void* Xt, const
   if (geom) { geom->NP = p.NP; geom->S = p.S; geom->NSET = C::NSET; }
   if (z_mode == 2 && topk_k <= 5) {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-    tc_fwd_kernel<G, K, 5><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_fwd_kernel<G, K, 5>, dim3(grid), dim3(C::THREADS), C::SMEM, st, tmW, tmY, p));
   } else if (z_mode == 2) {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-    tc_fwd_kernel<G, K, 8><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_fwd_kernel<G, K, 8>, dim3(grid), dim3(C::THREADS), C::SMEM, st, tmW, tmY, p));
   } else if (z_mode == 1) {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-    tc_fwd_kernel<G, K, -1><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_fwd_kernel<G, K, -1>, dim3(grid), dim3(C::THREADS), C::SMEM, st, tmW, tmY, p));
   } else {
     HASTE_CUDA_TRY(cudaFuncSetAttribute(tc_fwd_kernel<G, K, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-    tc_fwd_kernel<G, K, 0><<<grid, C::THREADS, C::SMEM, st>>>(tmW, tmY, p);
+    HASTE_CUDA_TRY(launch_pdl(tc_fwd_kernel<G, K, 0>, dim3(grid), dim3(C::THREADS), C::SMEM, st, tmW, tmY, p));
   }
   HASTE_LAUNCH_CHECK();
   return HASTE_OK;

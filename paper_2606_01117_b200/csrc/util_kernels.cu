@@ -15,6 +15,8 @@ __global__ void transpose_pad_kernel(const T* __restrict__ X, T* __restrict__ Xt
   __shared__ T tile[32][33];
   const int f0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
   const int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+  pdl_wait();
+  pdl_trigger();
 #pragma unroll
   for (int r = ty; r < 32; r += 8) {
     const int b = b0 + r, f = f0 + tx;
@@ -33,23 +35,32 @@ __global__ void transpose_pad_kernel(const T* __restrict__ X, T* __restrict__ Xt
 int launch_transpose_pad(haste_dtype_t dt, const void* X, void* Xt, int B, int d, int Bpad, int Bzero, cudaStream_t st) {
   dim3 grid(ceil_div(d, 32), ceil_div(Bzero, 32)), block(32, 8);
   if (dt == HASTE_F32)
-    transpose_pad_kernel<float><<<grid, block, 0, st>>>((const float*)X, (float*)Xt, B, d, Bpad, Bzero);
+    HASTE_CUDA_TRY(launch_pdl(transpose_pad_kernel<float>, grid, block, 0, st, (const float*)X, (float*)Xt, B, d, Bpad, Bzero));
   else
-    transpose_pad_kernel<bf16><<<grid, block, 0, st>>>((const bf16*)X, (bf16*)Xt, B, d, Bpad, Bzero);
-  HASTE_LAUNCH_CHECK();
+    HASTE_CUDA_TRY(launch_pdl(transpose_pad_kernel<bf16>, grid, block, 0, st, (const bf16*)X, (bf16*)Xt, B, d, Bpad, Bzero));
   return HASTE_OK;
 }
 
-// dX[b][f] (=|+=) dXt[f][b]
-__global__ void untranspose_f32_kernel(const float* __restrict__ dXt, float* __restrict__ dX, int B, int d, int Bpad,
+// dX[b][f] (=|+=) dXt[f][b]; what is read from dXt is zeroed behind it, so the workspace is clean for the next backward
+// pass without a memset between that pass's kernels (haste_api.cu keeps a host flag for the passes that end early)
+__global__ void untranspose_f32_kernel(float* __restrict__ dXt, float* __restrict__ dX, int B, int d, int Bpad,
                                        int accumulate) {
   __shared__ float tile[32][33];
   const int b0 = blockIdx.x * 32, f0 = blockIdx.y * 32;
   const int tx = threadIdx.x, ty = threadIdx.y;
+  pdl_wait();
+  pdl_trigger();
+  float v[4];
 #pragma unroll
-  for (int r = ty; r < 32; r += 8) {
-    const int f = f0 + r, b = b0 + tx;
-    tile[r][tx] = (f < d && b < B) ? dXt[(int64_t)f * Bpad + b] : 0.f;
+  for (int i = 0; i < 4; ++i) {       // all four loads first: the stores behind them may alias as far as the compiler knows
+    const int f = f0 + ty + 8 * i, b = b0 + tx;
+    v[i] = (f < d && b < B) ? __ldcg(dXt + (int64_t)f * Bpad + b) : 0.f;
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int f = f0 + ty + 8 * i, b = b0 + tx;
+    if (f < d && b < B) dXt[(int64_t)f * Bpad + b] = 0.f;
+    tile[ty + 8 * i][tx] = v[i];
   }
   __syncthreads();
 #pragma unroll
@@ -64,10 +75,9 @@ __global__ void untranspose_f32_kernel(const float* __restrict__ dXt, float* __r
   }
 }
 
-int launch_untranspose_f32(const float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st) {
+int launch_untranspose_f32(float* dXt, float* dX, int B, int d, int Bpad, int accumulate, cudaStream_t st) {
   dim3 grid(ceil_div(B, 32), ceil_div(d, 32)), block(32, 8);
-  untranspose_f32_kernel<<<grid, block, 0, st>>>(dXt, dX, B, d, Bpad, accumulate);
-  HASTE_LAUNCH_CHECK();
+  HASTE_CUDA_TRY(launch_pdl(untranspose_f32_kernel, grid, block, 0, st, dXt, dX, B, d, Bpad, accumulate));
   return HASTE_OK;
 }
 
