@@ -69,7 +69,10 @@ template <int G, int K, bool F32, bool SGD = false> struct DwCfg {
   static constexpr int NST = NST_RAW > 8 ? 8 : NST_RAW;
   // producer completion lag: LAG + 1 k-blocks of cp.async in flight per producer warp.  A narrow group's k-block is the same
   // gather for a fraction of the labels, so there the gather's latency is what bounds the kernel: more in flight
-  static constexpr int LAG = (G <= 16 && NST >= 7) ? 4 : 2;
+  static constexpr int LAG = 2;
+  // narrow groups: each producer warp gathers every fourth k-block whole (all K rows), as in the forward (tc_tail.cu,
+  // FwdCfg::NARROW): its wait / issue / wait-for-copies / fence / arrive chain is then on the critical path a quarter as often
+  static constexpr bool ROT = G <= 16;
   static constexpr int TS = N <= 128 ? 128 : 256;           // TMEM columns per accumulator slot
   static constexpr int OFF_EPI = NST * STAGE;
   static constexpr int OFF_BAR = OFF_EPI + EPI_BYTES;
@@ -110,7 +113,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   const int n_my = NGV > blockIdx.x ? (int)((NGV - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;     // groups of this CTA
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], 5); mbar_init(&empty[i], 1); }
+    for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], C::ROT ? 2 : 5); mbar_init(&empty[i], 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&t_full[i], 1); mbar_init(&t_empty[i], 4); }
     fence_barrier_init();
   }
@@ -132,8 +135,54 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   if (warp >= 4 && warp < 8) {
     // ===================== gather producers =====================
     const int pw = warp - 4;
-    constexpr int RPW = C::KV / 4;                   // slots per producer warp
     const int sub = lane >> 3, c = lane & 7;         // 4 rows per instruction, 8 chunks of 16 B per row
+    if constexpr (C::ROT) {
+      // k-blocks it = pw, pw + 4, ... of this CTA's sequence (group i = it / NKB, k-block kb = it % NKB); lane holds slots
+      // lane + 32 t of the current group's idx row; two k-blocks of copies in flight per warp
+      constexpr int NI = K / 32;
+      int idx_cur[NI];
+#pragma unroll
+      for (int t = 0; t < NI; ++t) idx_cur[t] = 0;
+      int i_cur = -1, prev_st = -1;
+      const int n_it = n_my * p.NKB;
+      for (int it = pw; it < n_it; it += 4) {
+        const int i = it / p.NKB, kb = it - i * p.NKB;
+        if (i != i_cur) {
+          i_cur = i;
+          const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+#pragma unroll
+          for (int t = 0; t < NI; ++t) idx_cur[t] = __ldg(p.idx + g * K + lane + 32 * t);
+        }
+        const int st = it % C::NST;
+        mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
+        const uint32_t dst0 = sbase + st * C::STAGE;
+        const bf16* src0 = p.Xt + kb * 128 + c * 8;
+#pragma unroll
+        for (int r4 = 0; r4 < K / 4; ++r4) {
+          const int row = 4 * r4 + sub;
+          const int f = __shfl_sync(0xffffffffu, idx_cur[(4 * r4) >> 5], row & 31);
+          const uint32_t dst = dst0 + row * 128 + (((uint32_t)(c ^ (row & 7))) << 4);
+          const bf16* src = src0 + (size_t)f * p.Bpad;
+          cp_async16(dst, src);
+          cp_async16(dst + C::HH_BYTES, src + 64);
+        }
+        cp_async_commit();
+        if (prev_st >= 0) {
+          cp_async_wait<1>();
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&full[prev_st]);
+        }
+        prev_st = st;
+      }
+      if (prev_st >= 0) {
+        cp_async_wait<0>();
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[prev_st]);
+      }
+    } else {
+    constexpr int RPW = C::KV / 4;                   // slots per producer warp
     // slot (pw*RPW + lane) of virtual group v is idx[v*KV + slot]; the second half of an unpaired last virtual group
     // (no group 2v+1) re-reads the first half's indices: its dY is zero-filled, its output rows are clipped
     auto idx_of = [&](int64_t v) -> int {
@@ -181,6 +230,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
         __syncwarp();
         if (lane == 0) mbar_arrive(&full[T % C::NST]);
       }
+    }
     }
   } else if (warp == 8) {
     // ===================== MMA issuer =====================
