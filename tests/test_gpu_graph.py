@@ -58,3 +58,53 @@ def test_step_captures_into_a_cuda_graph(shape):
         assert torch.equal(out[k], ref[k]), k
     for k in ("dX", "dXh"):
         assert torch.allclose(out[k], ref[k], rtol=1e-4, atol=1e-6), k
+
+
+def test_back_to_back_steps_are_reproducible():
+    """The step's kernels are launched with programmatic stream serialization (common.cuh): each starts while the one
+    before is still draining and must not touch global memory before its griddepcontrol.wait.  A kernel that did would
+    read a half-written dY, X^T or dX^T now and then.  40 steps back to back with inputs that change from step to step
+    (so that a stale read is a different value), each compared with the same step run alone: loss, dY, dW, db bit for
+    bit, dX up to the order of its float atomics -- and the workspace the transpose-out kernel zeroes behind itself
+    must be clean every time (dX would accumulate otherwise)."""
+    from paper_2606_01117_b200 import haste
+    from gpu_util import dev, to_dev, t32
+    B, d, L, G, K, Lh = 512, 768, 64 * 1200 + 7, 64, 128, 2048
+    inp = synth.small_case(77, B, d, L, G, K, dtype="bf16", with_bias=True)
+    W, idx, bias = to_dev(inp, "W"), t32(inp.idx), t32(inp.bias)
+    rowptr, col = t32(inp.rowptr), t32(inp.col)
+    layer = haste.HasteLayer(d, L, G, K, B, "bf16", flags=haste.HASTE_XT_FROM_FORWARD)
+    head = haste.HasteHead(d, Lh, B, "bf16", label_offset=0)
+    g = torch.Generator(device="cpu").manual_seed(5)
+    Xs = [(torch.randn(B, d, generator=g) * (0.5 + 0.25 * i)).to(torch.bfloat16).to(dev()) for i in range(4)]
+    Wh = (torch.randn(Lh, d, generator=g) * 0.02).to(torch.bfloat16).to(dev())
+
+    def new_out():
+        return dict(loss=torch.zeros(2, device=dev()), dY=layer.alloc_dy(B), dW=torch.empty(L, K, dtype=torch.bfloat16, device=dev()),
+                    db=torch.empty(L, device=dev()), dX=torch.empty(B, d, device=dev()),
+                    dYh=torch.empty(B, Lh, dtype=torch.bfloat16, device=dev()), dWh=torch.empty(Lh, d, dtype=torch.bfloat16, device=dev()),
+                    dXh=torch.empty(B, d, device=dev()))
+
+    def step(X, o):
+        layer.forward_loss(B, X, idx, W, bias, rowptr, col, loss=o["loss"][0:1], dY=o["dY"])
+        layer.backward(B, X, idx, W, o["dY"], dW=o["dW"], dbias=o["db"], dX=o["dX"])
+        head.forward_loss(B, X, Wh, None, rowptr, col, loss=o["loss"][1:2], dY=o["dYh"])
+        head.backward(B, X, Wh, o["dYh"], dWh=o["dWh"], dbias=None, dX=o["dXh"])
+
+    refs = []
+    for X in Xs:                                  # each step alone, a synchronize on both sides
+        o = new_out()
+        torch.cuda.synchronize()
+        step(X, o)
+        torch.cuda.synchronize()
+        refs.append(o)
+    outs = [new_out() for _ in range(4)]
+    torch.cuda.synchronize()
+    for it in range(40):                          # back to back, no synchronize: kernels of neighbouring steps overlap
+        step(Xs[it % 4], outs[it % 4])
+    torch.cuda.synchronize()
+    for i in range(4):
+        for k in ("loss", "dY", "dW", "db", "dYh", "dWh"):
+            assert torch.equal(outs[i][k], refs[i][k]), (i, k)
+        for k in ("dX", "dXh"):
+            assert torch.allclose(outs[i][k], refs[i][k], rtol=1e-4, atol=1e-6), (i, k)
