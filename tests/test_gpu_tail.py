@@ -329,3 +329,22 @@ def test_xt_from_forward_flag(oracle, H):
     b.layer.forward_loss(B, to_dev(inp2, "X"), b.idx, b.W, b.bias, b.rowptr, b.col, loss=None, dY=b.layer.alloc_dy(B))
     bb2 = b.backward()
     assert np.array_equal(bb2["dW"], bb["dW"])
+
+
+@pytest.mark.parametrize("shape", [(5000, 256, 64 * 37 + 5, 64, 64), (4100, 192, 16 * 90 + 3, 16, 64), (20000, 128, 32 * 9, 32, 64)],
+                         ids=lambda s: "B%d_d%d_L%d_G%d_K%d" % s)
+def test_large_batch(oracle, H, shape):
+    """Batches of many 128-row tiles: 40 tile pairs in the forward, 40 and 33 batch tiles x few group stripes in dX, and
+    (B = 20000) more batch tiles than SMs, where the tcgen05 dX kernel declines and the CUDA-core one runs; the transposes'
+    grids span several waves (they release their dependent kernel only when the last wave runs)."""
+    from gpu_util import TailRun
+    B, d, L, G, K = shape
+    inp = synth.small_case(9, B, d, L, G, K, dtype="bf16", with_bias=True, w_std=0.05)
+    run = TailRun(inp, G, flags=H.HASTE_IDX_SORTED_DISTINCT)
+    assert run.layer.kernel_family == 1
+    out = run.forward()
+    ref = oracle.tail_forward(inp.X, inp.idx, inp.W, inp.bias, inp.rowptr, inp.col, G)
+    _check_forward(oracle, out, ref, TOL["bf16"], inp)
+    bout = run.backward()
+    bref = oracle.tail_backward(inp.X, inp.idx, inp.W, ref["dY"], G)
+    _check_backward(oracle, bout, bref, TOL["bf16"], G)
