@@ -33,6 +33,8 @@ struct HeadParams {
   float* loss;                // FWD: device scalar, written by the last CTA
   float* logits;              // FWD: [B][L] fp32 or null
   float* dbias;               // DW: [L] or null
+  float4* zero;               // DW: a buffer this kernel zeroes on the side (the dX the next kernel reduces into), or null
+  int64_t zero_n;             //     its length in float4
   int write_out;              // FWD: dY; DW: dW_h
   float s;
 };
@@ -117,6 +119,10 @@ tc_head_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   tc_fence_after();
   pdl_wait();       // nothing above touches global memory (common.cuh, PDL)
   pdl_trigger();
+  if (MODE == HEAD_DW && p.zero) {      // no memset between this kernel and the dX kernel that follows it (PDL chain)
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < p.zero_n; e += (int64_t)gridDim.x * blockDim.x)
+      p.zero[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == 5) {
@@ -654,6 +660,7 @@ int tc_head_forward(TcHeadState* s, const HeadShape& sh, const void* X, const vo
 int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const void* Wh, const void* dY, void* dWh,
                      float* dbias, float* dX, int accumulate_dX, int deterministic, cudaStream_t st, int* n_launches) {
   *n_launches = 0;
+  bool dx_zeroed = false;
   if (dWh || dbias) {
     CUtensorMap tmA, tmB, tmO;
     int rc = map2d(&tmA, 2, dY, sh.L, sh.B, 64, 64);
@@ -663,12 +670,16 @@ int tc_head_backward(TcHeadState* s, const HeadShape& sh, const void* X, const v
     HeadParams p = base_params(sh);
     p.MT = ceil_div(sh.L, 128); p.NTL = dWh ? ceil_div(sh.d, HeadCfg<HEAD_DW>::BN) : 1; p.KB = ceil_div(sh.B, 64);
     p.dbias = dbias; p.write_out = dWh ? 1 : 0;
+    if (dX && !accumulate_dX && ((size_t)sh.B * sh.d) % 4 == 0 && (reinterpret_cast<uintptr_t>(dX) & 15u) == 0) {      // the dW kernel zeroes dX for the dX kernel
+      p.zero = reinterpret_cast<float4*>(dX); p.zero_n = (int64_t)sh.B * sh.d / 4;
+      dx_zeroed = true;
+    }
     rc = launch_head<HEAD_DW>(s, tmA, tmB, tmO, p, st);
     if (rc) return rc;
     ++*n_launches;
   }
   if (dX) {
-    if (!accumulate_dX) HASTE_CUDA_TRY(cudaMemsetAsync(dX, 0, (size_t)sh.B * sh.d * sizeof(float), st));
+    if (!accumulate_dX && !dx_zeroed) HASTE_CUDA_TRY(cudaMemsetAsync(dX, 0, (size_t)sh.B * sh.d * sizeof(float), st));
     CUtensorMap tmA, tmB, tmO;
     int rc = map2d(&tmA, 2, dY, sh.L, sh.B, 64, 128);
     if (!rc) rc = map2d(&tmB, 2, Wh, sh.d, sh.L, 64, 64);
