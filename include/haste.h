@@ -137,6 +137,21 @@ int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* 
 int haste_forward_topk(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W,
                        const float* bias /* [L] fp32 or NULL */, int k, float* out_val, int64_t* out_idx, void* stream);
 
+/* haste_forward_topk without any allocation in the call (for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  Same arguments, same results.  The candidate lists of the
+ * forward kernel live in a file-scope device array of the library image instead of a workspace the first call
+ * allocates: 4.625 MiB (the lists of at most 148 CTAs x 4 epilogue sets x 128 rows x 8 candidates, logits + labels), held
+ * by every GPU that loads the library until the process exits.  Its device address is looked up once per device inside
+ * haste_create; this call does no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   - A device with more than 148 SMs needs longer lists than the array holds: HASTE_ERR_UNSUPPORTED, nothing launched
+ *     (use haste_forward_topk there).
+ *   - ONE array per device, shared by every handle and every call: two calls that overlap on the GPU (different streams,
+ *     or different handles on one device) race on it.  Calls on one stream are ordered and safe.
+ *   - The array keeps the last call's contents; nothing in it needs clearing between calls (the forward kernel writes
+ *     every list the merge kernel of the same call reads). */
+int haste_forward_topk_static(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W,
+                              const float* bias /* [L] fp32 or NULL */, int k, float* out_val, int64_t* out_idx, void* stream);
+
 /* Backward from a dY in the library layout. */
 int haste_backward(haste_layer_t* h, int B,
                    const void* X, const int32_t* idx, const void* W, const void* dY,

@@ -4,6 +4,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 #include <new>
 
@@ -75,6 +76,34 @@ struct Profiler {
 
 static inline size_t esize(haste_dtype_t dt) { return dt == HASTE_F32 ? 4 : 2; }
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// ---- scratch of haste_forward_topk_static: the candidate lists of the fused top-k forward in device memory that belongs
+// to the library image, so that the call allocates nothing.  [2][TOPK_STATIC_ENTRIES] 32-bit words: candidate logits
+// (fp32), then candidate labels (int32), each [CTAs <= 148][4 epilogue sets][128 rows][8 candidates] = 4.625 MiB in all,
+// held by every GPU that loads the library until the process exits.  ONE array per device: every call on that device
+// shares it (calls that overlap on the GPU race), and it keeps the last call's contents -- nothing in it has to start at
+// zero, because the forward kernel writes every list its merge kernel reads (tc_tail.cu, end of the top-k epilogue).
+// In host code the NAME below is a host-side stand-in, not a device address: the address is asked for once per device
+// (resolve_topk_static, called from haste_create with that device current) and that pointer is what the kernels get.
+static constexpr int TOPK_STATIC_MAX_CTAS = 148;
+static constexpr size_t TOPK_STATIC_ENTRIES = (size_t)TOPK_STATIC_MAX_CTAS * 4 * 128 * 8;
+static __device__ __align__(256) unsigned char g_topk_static[2 * TOPK_STATIC_ENTRIES * 4];
+static constexpr int TOPK_STATIC_MAX_DEVICES = 64;
+struct TopkStaticDev { void* ptr; cudaError_t err; bool tried; };
+static TopkStaticDev g_topk_static_dev[TOPK_STATIC_MAX_DEVICES] = {};
+static std::mutex g_topk_static_mu;
+// `device` must be the current device.  Never fails the caller: the outcome is kept for haste_forward_topk_static.
+static void resolve_topk_static(int device) {
+  if (device < 0 || device >= TOPK_STATIC_MAX_DEVICES) return;
+  std::lock_guard<std::mutex> lock(g_topk_static_mu);
+  TopkStaticDev& e = g_topk_static_dev[device];
+  if (e.tried) return;
+  void* ptr = nullptr;
+  e.err = cudaGetSymbolAddress(&ptr, g_topk_static);
+  e.ptr = e.err == cudaSuccess ? ptr : nullptr;
+  e.tried = true;
+  if (e.err != cudaSuccess) (void)cudaGetLastError();      // not sticky; reported by the entry point that needs it
+}
 
 }  // namespace haste
 
@@ -220,6 +249,7 @@ int haste_create(haste_layer_t** out, const haste_config_t* cfg, int cuda_device
       return HASTE_ERR_NOMEM;
     }
   }
+  resolve_topk_static(cuda_device);      // set-up of haste_forward_topk_static (this device is current here)
   *out = h;
   return HASTE_OK;
 }
@@ -396,6 +426,67 @@ int haste_forward_topk(haste_layer_t* h, int B, const void* X, const int32_t* id
                        &geom, st, &n);
   if (rc) return rc;
   rc = launch_topk_merge(h->topk_val, h->topk_idx, geom.NP, geom.S, geom.NSET, ceil_div(B, 128), B, k, h->cfg.label_offset, out_val,
+                         out_idx, st);
+  if (rc) return rc;
+  pf.end(HASTE_KERNEL_FORWARD, st);
+  h->last_launches = n + 2;
+  return HASTE_OK;
+}
+
+int haste_forward_topk_static(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias, int k,
+                              float* out_val, int64_t* out_idx, void* stream) {
+  int rc = check_call(h, B, "haste_forward_topk_static");
+  if (rc) return rc;
+  if (!X || !idx || !W || !out_val || !out_idx) { set_error("haste_forward_topk_static: X, idx, W, out_val and out_idx are required"); return HASTE_ERR_INVALID_ARG; }
+  if (k < 1 || k > 8) { set_error("haste_forward_topk_static: k must be in [1, 8]"); return HASTE_ERR_INVALID_ARG; }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(idx)) { set_error("haste_forward_topk_static: X, W and idx must be 16-byte aligned"); return HASTE_ERR_INVALID_ARG; }
+  if (h->family != 1) { set_error("haste_forward_topk_static: only the tcgen05 kernel family has the fused top-k forward"); return HASTE_ERR_UNSUPPORTED; }
+  // the forward kernel's grid is at most one CTA per SM, four epilogue sets of 128 rows x 8 candidates each
+  const size_t need = (size_t)tc_tail_num_sms(h->tc) * 4 * 128 * 8;
+  if (need > TOPK_STATIC_ENTRIES) {
+    set_error("haste_forward_topk_static: this device has %d SMs, the static scratch holds the candidate lists of at most %d CTAs "
+              "(%zu bytes); use haste_forward_topk", tc_tail_num_sms(h->tc), TOPK_STATIC_MAX_CTAS, sizeof(g_topk_static));
+    return HASTE_ERR_UNSUPPORTED;
+  }
+  if (h->device < 0 || h->device >= TOPK_STATIC_MAX_DEVICES) {
+    set_error("haste_forward_topk_static: device index %d beyond the %d devices the static scratch is tracked for", h->device, TOPK_STATIC_MAX_DEVICES);
+    return HASTE_ERR_UNSUPPORTED;
+  }
+  float* cand_val = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_topk_static_mu);
+    const TopkStaticDev& e = g_topk_static_dev[h->device];
+    if (!e.tried || !e.ptr) {
+      set_error("haste_forward_topk_static: the address of the static scratch is not known on device %d (cudaGetSymbolAddress: %s)",
+                h->device, e.tried ? cudaGetErrorString(e.err) : "not asked for");
+      return HASTE_ERR_CUDA;
+    }
+    cand_val = static_cast<float*>(e.ptr);
+  }
+  int* cand_idx = reinterpret_cast<int*>(cand_val + TOPK_STATIC_ENTRIES);
+  DeviceGuard guard(h->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const TailShape sh = make_shape(h, B);
+  Profiler& pf = *h->prof;
+  h->last_launches = 0;
+  if (B == 0) return HASTE_OK;
+  if (h->NG == 0) {     // no labels: every slot empty
+    HASTE_CUDA_TRY(cudaMemsetAsync(out_idx, 0xff, (size_t)B * k * 8, st));
+    HASTE_CUDA_TRY(cudaMemsetAsync(out_val, 0xff, (size_t)B * k * 4, st));
+    return HASTE_OK;
+  }
+  pf.begin(HASTE_KERNEL_PREP_FWD, st);
+  rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+  if (rc) return rc;
+  pf.end(HASTE_KERNEL_PREP_FWD, st);
+  int n = 0;
+  TopkGeom geom;
+  geom.k = k;
+  pf.begin(HASTE_KERNEL_FORWARD, st);
+  rc = tc_tail_forward(h->tc, sh, h->Xt, idx, W, bias, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 2, cand_val, cand_idx,
+                       &geom, st, &n);
+  if (rc) return rc;
+  rc = launch_topk_merge(cand_val, cand_idx, geom.NP, geom.S, geom.NSET, ceil_div(B, 128), B, k, h->cfg.label_offset, out_val,
                          out_idx, st);
   if (rc) return rc;
   pf.end(HASTE_KERNEL_FORWARD, st);

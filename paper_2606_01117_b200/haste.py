@@ -20,7 +20,7 @@ HASTE_OK, HASTE_ERR_INVALID_ARG, HASTE_ERR_BAD_INDEX, HASTE_ERR_UNSUPPORTED, HAS
 
 # Every symbol include/haste.h declares (tests check the library exports all of them).
 SYMBOLS = [
-    "haste_create", "haste_destroy", "haste_dy_bytes", "haste_validate_index", "haste_forward_loss", "haste_forward_logits", "haste_forward_topk",
+    "haste_create", "haste_destroy", "haste_dy_bytes", "haste_validate_index", "haste_forward_loss", "haste_forward_logits", "haste_forward_topk", "haste_forward_topk_static",
     "haste_backward", "haste_backward_sgd", "haste_rewire", "haste_dy_unpack", "haste_dy_pack", "haste_head_create", "haste_head_destroy",
     "haste_head_forward_loss", "haste_head_backward", "haste_status_string", "haste_last_error",
     "haste_kernel_family", "haste_head_kernel_family", "haste_last_launch_count", "haste_head_last_launch_count",
@@ -64,6 +64,7 @@ def lib():
     L.haste_forward_loss.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.haste_forward_logits.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     L.haste_forward_topk.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]
+    L.haste_forward_topk_static.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]
     L.haste_backward.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     L.haste_backward_sgd.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, vp, i32, vp]
     L.haste_rewire.argtypes = [vp, vp, vp, vp, f32, i32, ctypes.c_uint64, i32, ctypes.POINTER(ctypes.c_int64), vp]
@@ -168,6 +169,12 @@ class HasteLayer:
     def forward_topk(self, B, X, idx, W, bias, k, out_val, out_idx, stream=None):
         _check(lib().haste_forward_topk(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(bias), k, _ptr(out_val), _ptr(out_idx),
                                         _stream(stream)))
+
+    def forward_topk_static(self, B, X, idx, W, bias, k, out_val, out_idx, stream=None):
+        """haste_forward_topk_static: the same results with the candidate lists in the library's static device array; the
+        call allocates nothing (include/haste.h)."""
+        _check(lib().haste_forward_topk_static(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(bias), k, _ptr(out_val),
+                                               _ptr(out_idx), _stream(stream)))
 
     def forward_logits(self, B, X, idx, W, bias, Z, stream=None):
         _check(lib().haste_forward_logits(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(bias), _ptr(Z), _stream(stream)))
