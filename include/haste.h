@@ -118,6 +118,17 @@ int haste_forward_loss(haste_layer_t* h, int B,
                        float* logits_out,         /* optional [B,L] row-major fp32, or NULL                   */
                        void* stream);
 
+/* Forward + fused BCE AND the weight gradient in one call (the first slice of the single-pass step):
+ * exactly haste_forward_loss(..., logits_out = NULL) followed by haste_backward(..., dW, dbias, dX = NULL) -- the same
+ * loss, dY, dW (in the handle's dw_dtype) and dbias, with the same argument meanings, layouts and ownership.  dY is
+ * required (the input-gradient step, haste_backward with dX only, still reads it).  For bf16 handles with G = 64,
+ * K in {64, 128} and B <= 512 this is ONE kernel in which the gathered tile X[:, idx_g] and the dY tile just produced are
+ * still on chip when the weight-gradient contraction runs: dY is written once and never read back, X^T is gathered
+ * once.  Every other shape runs the two calls one after the other.  X, idx, W, dY, dW 16-byte aligned. */
+int haste_forward_loss_dw(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias,
+                          const int32_t* tgt_rowptr, const int32_t* tgt_col, float* loss, void* dY,
+                          void* dW /* [L,K] dw_dtype or NULL */, float* dbias /* [L] fp32 or NULL */, void* stream);
+
 /* Logits-only forward (z = <w_l, h_I> per label; the inference pass behind Eq. 4):
  * Z receives z[i,l] = bias[l] + sum_j W[l,j] X[i, idx[l/G, j]] rounded to `dtype`, in the library's dY layout
  * ([NG][B][G], haste_dy_bytes(h,B) bytes, padding labels >= L written as zero; haste_dy_unpack converts it to

@@ -355,6 +355,55 @@ int haste_forward_loss(haste_layer_t* h, int B, const void* X, const int32_t* id
   return HASTE_OK;
 }
 
+int haste_forward_loss_dw(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias,
+                          const int32_t* tgt_rowptr, const int32_t* tgt_col, float* loss, void* dY, void* dW, float* dbias,
+                          void* stream) {
+  int rc = check_call(h, B, "haste_forward_loss_dw");
+  if (rc) return rc;
+  if (!X || !idx || !W || !dY) { set_error("haste_forward_loss_dw: X, idx, W and dY are required"); return HASTE_ERR_INVALID_ARG; }
+  if ((tgt_rowptr == nullptr) != (tgt_col == nullptr)) {
+    set_error("haste_forward_loss_dw: tgt_rowptr and tgt_col must both be given or both be NULL");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (!aligned16(X) || !aligned16(W) || !aligned16(dY) || !aligned16(idx) || !aligned16(dW)) {
+    set_error("haste_forward_loss_dw: X, W, idx, dY and dW must be 16-byte aligned");
+    return HASTE_ERR_INVALID_ARG;
+  }
+  if (h->family == 1 && B > 0 && h->NG > 0 && h->cfg.G == 64 && B <= 512 && (dW || dbias)) {
+    DeviceGuard guard(h->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const TailShape sh = make_shape(h, B);
+    Profiler& pf = *h->prof;
+    h->last_launches = 0;
+    pf.begin(HASTE_KERNEL_PREP_FWD, st);
+    rc = launch_transpose_pad(h->cfg.dtype, X, h->Xt, B, sh.d, h->Bpad, round_up(B, 128), st);
+    if (rc) return rc;
+    h->last_launches++;
+    pf.end(HASTE_KERNEL_PREP_FWD, st);
+    int n = 0;
+    pf.begin(HASTE_KERNEL_FORWARD, st);
+    rc = tc_tail_forward_dw(h->tc, sh, h->Xt, idx, W, bias, tgt_rowptr, tgt_col, loss ? h->partials : nullptr, loss, dY, dW, dbias, st, &n);
+    if (rc == HASTE_OK) {
+      pf.end(HASTE_KERNEL_FORWARD, st);
+      h->last_launches += n;
+      return HASTE_OK;
+    }
+    if (rc != HASTE_ERR_UNSUPPORTED) return rc;
+  }
+  // every other shape: the two calls this one is defined as
+  rc = haste_forward_loss(h, B, X, idx, W, bias, tgt_rowptr, tgt_col, loss, dY, nullptr, stream);
+  if (rc) return rc;
+  const int n_fwd = h->last_launches;
+  if (dW || dbias) {
+    rc = haste_backward(h, B, X, idx, W, dY, dW, dbias, nullptr, 0, stream);
+    if (rc) return rc;
+  } else {
+    h->last_launches = 0;
+  }
+  h->last_launches += n_fwd;
+  return HASTE_OK;
+}
+
 int haste_forward_logits(haste_layer_t* h, int B, const void* X, const int32_t* idx, const void* W, const float* bias, void* Z,
                          void* stream) {
   int rc = check_call(h, B, "haste_forward_logits");

@@ -25,6 +25,11 @@ int tc_tail_forward(TcTailState* s, const TailShape& sh, const void* Xt, const i
 // z_mode = 2: fused top-k; topk_val / topk_idx: [grid][sets][128][8] candidate workspace (grid <= num SMs, sets <= 4)
 int tc_tail_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* dW,
                float* dbias, cudaStream_t st, int* n_launches);
+// forward + loss + dY AND the weight gradient in one kernel (tc_fused.cu): G = 64, K in {64, 128}, B <= 512; otherwise
+// HASTE_ERR_UNSUPPORTED with nothing launched
+int tc_tail_forward_dw(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* W, const float* bias,
+                       const int32_t* rowptr, const int32_t* col, float* loss_partials, float* loss, void* dY, void* dW,
+                       float* dbias, cudaStream_t st, int* n_launches);
 // dW with the SGD-momentum step of the output layer as its epilogue (tc_dw.cu): W, mom (and bias, bmom) updated in place
 int tc_tail_dw_sgd(TcTailState* s, const TailShape& sh, const void* Xt, const int32_t* idx, const void* dY, void* W, float* mom,
                    float* bias, float* bmom, float lr, float mu, float wd, cudaStream_t st, int* n_launches);

@@ -20,7 +20,7 @@ HASTE_OK, HASTE_ERR_INVALID_ARG, HASTE_ERR_BAD_INDEX, HASTE_ERR_UNSUPPORTED, HAS
 
 # Every symbol include/haste.h declares (tests check the library exports all of them).
 SYMBOLS = [
-    "haste_create", "haste_destroy", "haste_dy_bytes", "haste_validate_index", "haste_forward_loss", "haste_forward_logits", "haste_forward_topk", "haste_forward_topk_static",
+    "haste_create", "haste_destroy", "haste_dy_bytes", "haste_validate_index", "haste_forward_loss", "haste_forward_loss_dw", "haste_forward_logits", "haste_forward_topk", "haste_forward_topk_static",
     "haste_backward", "haste_backward_sgd", "haste_rewire", "haste_dy_unpack", "haste_dy_pack", "haste_head_create", "haste_head_destroy",
     "haste_head_forward_loss", "haste_head_backward", "haste_status_string", "haste_last_error",
     "haste_kernel_family", "haste_head_kernel_family", "haste_last_launch_count", "haste_head_last_launch_count",
@@ -62,6 +62,7 @@ def lib():
     L.haste_dy_bytes.restype = ctypes.c_size_t
     L.haste_validate_index.argtypes = [vp, vp, vp]
     L.haste_forward_loss.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.haste_forward_loss_dw.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.haste_forward_logits.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     L.haste_forward_topk.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]
     L.haste_forward_topk_static.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]
@@ -175,6 +176,10 @@ class HasteLayer:
         call allocates nothing (include/haste.h)."""
         _check(lib().haste_forward_topk_static(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(bias), k, _ptr(out_val),
                                                _ptr(out_idx), _stream(stream)))
+
+    def forward_loss_dw(self, B, X, idx, W, bias, rowptr, col, loss=None, dY=None, dW=None, dbias=None, stream=None):
+        _check(lib().haste_forward_loss_dw(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(bias), _ptr(rowptr), _ptr(col), _ptr(loss),
+                                           _ptr(dY), _ptr(dW), _ptr(dbias), _stream(stream)))
 
     def forward_logits(self, B, X, idx, W, bias, Z, stream=None):
         _check(lib().haste_forward_logits(self.h, B, _ptr(X), _ptr(idx), _ptr(W), _ptr(bias), _ptr(Z), _stream(stream)))
