@@ -550,6 +550,23 @@ def main():
         t = [layer.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nx)]
         extras["forward_topk_k5"] = {"ms": float(np.mean(t)), "ms_median": float(np.median(t)), "ms_min": float(np.min(t)),
                                      "note": "forward kernel with per-thread candidate lists + merge kernel; no [B,L] buffer"}
+        # forward + BCE + weight gradient in ONE kernel (haste_forward_loss_dw, first slice) beside the two
+        # kernels of the step that it stands for (`kernels.forward` + `kernels.dW`)
+        try:
+            for _ in range(2):
+                layer.forward_loss_dw(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY, dW=dW, dbias=db)
+            torch.cuda.synchronize()
+            for _ in range(nx):
+                layer.forward_loss_dw(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY, dW=dW, dbias=db)
+            torch.cuda.synchronize()
+            t = [layer.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nx)]
+            fb = L * K * esz + cfg.NG * K * 4 + B * d * esz + cfg.NG * G * B * esz + L * K * dW.element_size()
+            g = fb / (float(np.mean(t)) * 1e-3) / 1e9
+            extras["forward_dw_fused"] = {"ms": float(np.mean(t)), "ms_median": float(np.median(t)), "ms_min": float(np.min(t)), "alg_bytes": int(fb),
+                                          "GB/s": g, "frac_hbm": g / _peaks()["hbm"], "launches": int(layer.last_launch_count),
+                                          "note": "one kernel for forward + loss + dY + dW + db where it exists (G = 64, B <= 512), else the two kernels; dY written once, never read back"}
+        except haste.HasteError as e:
+            extras["forward_dw_fused"] = {"unsupported": str(e)}
     layer.set_profiling(0)
     if use_head:
         head.set_profiling(0)
