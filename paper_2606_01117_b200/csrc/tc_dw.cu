@@ -111,6 +111,10 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t NGV = C::PAIR ? (p.NG + 1) / 2 : p.NG;                                               // (virtual) groups
   const int n_my = NGV > blockIdx.x ? (int)((NGV - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;     // groups of this CTA
+  // ... taken from the LAST group down: the forward kernel before this one wrote dY in ascending group order, so the
+  // groups written last are the ones still in the 126 MB L2 (and the dX kernel after this one, ascending again, finds
+  // the groups this kernel read last)
+  auto group_of = [&](int i) -> int64_t { return NGV - 1 - (blockIdx.x + (int64_t)i * gridDim.x); };
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < C::NST; ++i) { mbar_init(&full[i], C::ROT ? 2 : 5); mbar_init(&empty[i], 1); }
@@ -149,7 +153,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
         const int i = it / p.NKB, kb = it - i * p.NKB;
         if (i != i_cur) {
           i_cur = i;
-          const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+          const int64_t g = group_of(i);
 #pragma unroll
           for (int t = 0; t < NI; ++t) idx_cur[t] = __ldg(p.idx + g * K + lane + 32 * t);
         }
@@ -191,12 +195,11 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
       return __ldg(p.idx + off);
     };
     int idx_cur = 0, idx_nxt = 0;
-    if (lane < RPW && n_my > 0) idx_nxt = idx_of(blockIdx.x);
+    if (lane < RPW && n_my > 0) idx_nxt = idx_of(group_of(0));
     int it = 0;
     for (int i = 0; i < n_my; ++i) {
-      const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
       idx_cur = idx_nxt;
-      if (lane < RPW && i + 1 < n_my) idx_nxt = idx_of(g + gridDim.x);
+      if (lane < RPW && i + 1 < n_my) idx_nxt = idx_of(group_of(i + 1));
       for (int kb = 0; kb < p.NKB; ++kb, ++it) {
         const int st = it % C::NST;
         mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
@@ -272,7 +275,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     if (lane == 0) {
       int it = 0;
       for (int i = 0; i < n_my; ++i) {
-        const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+        const int64_t g = group_of(i);
         for (int kb = 0; kb < p.NKB; ++kb, ++it) {
           const int st = it % C::NST;
           mbar_wait(&empty[st], ((it / C::NST) & 1) ^ 1);
@@ -298,7 +301,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
     constexpr int RWC = C::RW;
     const int rwv = C::PADM ? max(0, min(RWC, G - RWC * q)) : RWC;
     for (int i = 0; i < n_my; ++i) {
-      const int64_t g = blockIdx.x + (int64_t)i * gridDim.x;
+      const int64_t g = group_of(i);
       const int slot = i & 1;
       mbar_wait(&t_full[slot], (i >> 1) & 1);
       tc_fence_after();
@@ -320,7 +323,7 @@ tc_dw_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CU
         const int64_t l = l0 + lane;
         const bool own = lane < rwv && l < p.L;
         if (i + 1 < n_my) {
-          const int64_t ln0 = l0 + (int64_t)gridDim.x * C::GL;
+          const int64_t ln0 = l0 - (int64_t)gridDim.x * C::GL;      // the next group of this CTA
           constexpr int WL = K * 2 / 128, ML = K * 4 / 128;          // 128-byte lines per row of W / of the momentum
           for (int e = lane; e < rwv * (WL + ML); e += 32) {
             const int r = e / (WL + ML), b = e - r * (WL + ML);
