@@ -132,3 +132,40 @@ def test_forward_loss_dw_heavy_rows_and_trained_regime(oracle):
     assert oracle.rel_l2(got[rows, inp.col], ref["dY"][rows, inp.col]) <= 5e-3
     assert oracle.rel_l2(dW.cpu().numpy(), bref["dW"]) <= 5e-3
     assert oracle.rel_l2(db.cpu().numpy(), bref["db"]) <= 5e-3
+
+
+def test_forward_loss_dw_optional_arguments(oracle):
+    """dW alone, db alone, no loss, no targets, a label offset: each output must be what the full call gives."""
+    from paper_2606_01117_b200 import haste
+    from gpu_util import dev, to_dev, t32
+    B, d, L, G, K, off = 200, 256, 64 * 170 + 3, 64, 128, 5000
+    inp = synth.small_case(9, B, d, L, G, K, dtype="bf16", n_pos=4, with_bias=True, w_std=0.05)
+    col = (inp.col + off).astype(np.int32)
+    layer = haste.HasteLayer(d, L, G, K, B, "bf16", dw_dtype="f32", label_offset=off)
+    X, W, idx, bias = to_dev(inp, "X"), to_dev(inp, "W"), t32(inp.idx), t32(inp.bias)
+    rowptr, colt = t32(inp.rowptr), t32(col)
+
+    def call(want_loss=True, want_dw=True, want_db=True, targets=True):
+        loss = torch.full((1,), float("nan"), device=dev()) if want_loss else None
+        dY = layer.alloc_dy(B)
+        dW = torch.full((L, K), float("nan"), device=dev()) if want_dw else None
+        db = torch.full((L,), float("nan"), device=dev()) if want_db else None
+        layer.forward_loss_dw(B, X, idx, W, bias, rowptr if targets else None, colt if targets else None, loss=loss, dY=dY, dW=dW, dbias=db)
+        torch.cuda.synchronize()
+        return loss, dY, dW, db
+
+    loss, dY, dW, db = call()
+    ref = oracle.tail_forward(inp.X, inp.idx, inp.W, inp.bias, inp.rowptr, col, G, label_offset=off)
+    bref = oracle.tail_backward(inp.X, inp.idx, inp.W, ref["dY"], G)
+    assert abs(float(loss.item()) - ref["loss"]) <= 2e-5 * abs(ref["loss"])
+    assert oracle.rel_l2(dW.cpu().numpy(), bref["dW"]) <= 5e-3 and oracle.rel_l2(db.cpu().numpy(), bref["db"]) <= 5e-3
+    l2, dY2, dW2, db2 = call(want_loss=False, want_db=False)
+    assert db2 is None and torch.equal(dY2, dY) and torch.equal(dW2, dW)
+    l3, dY3, dW3, db3 = call(want_dw=False)
+    assert dW3 is None and torch.equal(dY3, dY) and torch.equal(db3, db) and float(l3.item()) == float(loss.item())
+    # no targets: every label is a negative
+    l4, dY4, dW4, db4 = call(targets=False)
+    ref4 = oracle.tail_forward(inp.X, inp.idx, inp.W, inp.bias, np.zeros(B + 1, dtype=np.int32), np.zeros(0, dtype=np.int32), G)
+    bref4 = oracle.tail_backward(inp.X, inp.idx, inp.W, ref4["dY"], G)
+    assert abs(float(l4.item()) - ref4["loss"]) <= 2e-5 * abs(ref4["loss"])
+    assert oracle.rel_l2(dW4.cpu().numpy(), bref4["dW"]) <= 5e-3 and oracle.rel_l2(db4.cpu().numpy(), bref4["db"]) <= 5e-3
