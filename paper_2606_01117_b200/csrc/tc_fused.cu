@@ -20,8 +20,8 @@
 // What bounds this kernel is how long an H stage lives: from its gather through the forward MMAs and the WHOLE epilogue of
 // the tile to the weight-gradient MMAs that read it last.  So a tile's epilogue is made short: EIGHT warps per tile (TMEM
 // lane quadrant x 32-label half; a thread does one batch row x 32 labels), two tiles in flight (tile T belongs to the
-// warps of parity T & 1), and the issuing warp serves two queues without ever sleeping on one of them: forward MMAs of the
-// next gathered tile, weight-gradient MMAs of the next tile whose dY is in shared memory.  The weight-gradient accumulator
+// warps of parity T & 1), and TWO issuing warps, one per queue: forward MMAs of the next gathered tile; weight-gradient
+// MMAs (and the dY store) of the next tile whose dY is in shared memory.  The weight-gradient accumulator
 // D_w [64 labels x K + 8] lives in TMEM across a group's tiles, one buffer per group parity, and is written out (dW_g,
 // db_g) by the warps of that parity a few tiles later.
 #include <algorithm>
@@ -77,7 +77,7 @@ template <int G, int K> struct FusedCfg {
   static constexpr int NBAR = 2 * HS + 2 * WS + 2 * NSLOT + 2 * NTS + 4;
   static constexpr int OFF_MISC = OFF_BAR + NBAR * 8;
   static constexpr int SMEM = OFF_MISC + 128 + 1024;
-  static constexpr int THREADS = (16 + 6) * 32;
+  static constexpr int THREADS = (16 + 7) * 32;              // 16 epilogue, 4 producers, 2 MMA issuers, 1 W loader
 };
 
 __device__ __forceinline__ uint32_t fz_tmem_ld1(uint32_t taddr) {
@@ -185,75 +185,66 @@ tc_fused_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__
       if (lane == 0) mbar_arrive(&h_full[(total - 1) % C::HS]);
     }
   } else if (warp == 20) {
-    // ===================== MMA issuer: two queues, never asleep on one of them =====================
+    // ===================== MMA issuer 1 of 2: the forward of every tile =====================
+    // (One issuing warp for both queues was measured to be this kernel's bottleneck: it never idled -- 18 idle polls in 280
+    // tiles -- while producers and epilogue warps waited 40-55 % of the time.  The two queues touch different accumulators
+    // and every hand-over goes through a commit, so they can be issued by two threads.)
     constexpr uint32_t idesc_f = make_idesc_bf16(128, G, /*A (H) MN-major*/ 1, /*B (W) K-major*/ 0);
-    constexpr uint32_t idesc_w = make_idesc_bf16(64, C::NW, /*A (dY tile) MN-major*/ 1, /*B (H) K-major*/ 0);
     const uint64_t fa0 = make_sdesc_sw128(sbase + C::OFF_H, C::HH_BYTES, 1024);   // leading offset: the second 64 batch columns
     const uint64_t fb0 = make_sdesc_sw128(sbase + C::OFF_W, 16, 1024);
+    int gl = 0, t = 0;
+    for (int T = 0; T < total; ++T) {
+      const int ws = gl % C::WS, hs = T % C::HS, slot = T % C::NSLOT;
+      if (t == 0) mbar_wait(&w_full[ws], (gl / C::WS) & 1);
+      mbar_wait(&h_full[hs], (T / C::HS) & 1);
+      mbar_wait(&t_empty[slot], ((T / C::NSLOT) & 1) ^ 1);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t ad0 = fa0 + (uint64_t)((hs * C::H_BYTES) >> 4);
+        const uint64_t bd0 = fb0 + (uint64_t)((ws * C::W_BYTES) >> 4);
+        const uint32_t d = tmem_base + C::T_FWD0 + slot * G;
+#pragma unroll
+        for (int j = 0; j < K / 16; ++j)
+          umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * (G * 128) + (j & 3) * 32) >> 4), idesc_f,
+                   j > 0 ? 1u : 0u);
+        umma_commit(&t_full[slot]);
+      }
+      __syncwarp();
+      if (++t == NT) { t = 0; ++gl; }
+    }
+  } else if (warp == 22) {
+    // ===================== MMA issuer 2 of 2: the weight gradient of every tile, and its dY store =====================
+    // The tile's forward MMAs have completed before this queue sees the tile (its dY exists), so the commits below, which
+    // track this thread's MMAs only, release the H stage and the W stage safely.
+    constexpr uint32_t idesc_w = make_idesc_bf16(64, C::NW, /*A (dY tile) MN-major*/ 1, /*B (H) K-major*/ 0);
     const uint64_t wa0 = make_sdesc_sw128(sbase + C::OFF_ST, 8192, 1024);         // [128 batch rows][64 labels], as stored
     const uint64_t wb0 = make_sdesc_sw128(sbase + C::OFF_H, 16, 1024);            // rows = slots (+ ones), 64 batch columns per m-block
-    int Tf = 0, glf = 0, tf = 0;        // next forward: tile, its group, its batch tile
-    int Tw = 0, glw = 0, tw = 0;        // next weight gradient
-    bool f_w = false, f_h = false, f_t = false, w_d = false, w_s = false;   // conditions already seen true
-    // (one answer for the whole warp: the elected lane issues inside warp-uniform branches)
-    auto ready = [](uint64_t* b, uint32_t parity) { return __all_sync(0xffffffffu, mbar_test_wait(b, parity)) != 0; };
-    while (Tw < total) {
-      // ---- weight gradient of tile Tw: its dY is staged (and, first tile of a group, the D_w buffer is written out)
-      if (!w_d) w_d = tw != 0 || ready(&dw_empty[glw & 1], ((glw >> 1) & 1) ^ 1);
-      if (!w_s) w_s = ready(&s_full[Tw & 1], (Tw >> 1) & 1);
-      if (w_d && w_s) {
-        tc_fence_after();
-        const int hs = Tw % C::HS, buf = glw & 1;
-        if (elect_one()) {
-          const uint64_t ad0 = wa0 + (uint64_t)(((Tw & 1) * C::ST_BYTES) >> 4);
-          const uint64_t bd0 = wb0 + (uint64_t)((hs * C::H_BYTES) >> 4);
-          const uint32_t d = tmem_base + buf * C::DW_COLS;
+    int glw = 0, tw = 0;
+    for (int Tw = 0; Tw < total; ++Tw) {
+      const int hs = Tw % C::HS, buf = glw & 1;
+      if (tw == 0) mbar_wait(&dw_empty[buf], ((glw >> 1) & 1) ^ 1);        // D_w buffer written out (two groups ago)
+      mbar_wait(&s_full[Tw & 1], (Tw >> 1) & 1);                             // the epilogue has staged this tile's dY
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t ad0 = wa0 + (uint64_t)(((Tw & 1) * C::ST_BYTES) >> 4);
+        const uint64_t bd0 = wb0 + (uint64_t)((hs * C::H_BYTES) >> 4);
+        const uint32_t d = tmem_base + buf * C::DW_COLS;
 #pragma unroll
-          for (int j = 0; j < 8; ++j)
-            umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * C::HH_BYTES + (j & 3) * 32) >> 4), idesc_w,
-                     (tw | j) ? 1u : 0u);
-          umma_commit(&h_empty[hs]);                    // (the tile's forward MMAs were issued before these)
-          umma_commit(&s_empty[Tw & 1]);
-          if (tw == NT - 1) { umma_commit(&dw_full[buf]); umma_commit(&w_empty[glw % C::WS]); }
-          // the same tile goes to HBM as dY (rows past the batch are clipped by the tensor map).  elect.sync names the same
-          // thread every time, so the bulk groups are this thread's: all but the newest store have been read -> the tile
-          // before this one may be overwritten as far as its store is concerned (second arrival on its s_empty)
-          tma_store_3d(&tmY, smem + C::OFF_ST + (Tw & 1) * C::ST_BYTES, 0, tw * 128, (int)(stripe + (int64_t)glw * S));
-          bulk_commit();
-          if (Tw >= 1) { bulk_wait_read<1>(); mbar_arrive(&s_empty[(Tw - 1) & 1]); }
-        }
-        __syncwarp();
-        w_d = w_s = false;
-        ++Tw;
-        if (++tw == NT) { tw = 0; ++glw; }
-        continue;
+        for (int j = 0; j < 8; ++j)
+          umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * C::HH_BYTES + (j & 3) * 32) >> 4), idesc_w,
+                   (tw | j) ? 1u : 0u);
+        umma_commit(&h_empty[hs]);
+        umma_commit(&s_empty[Tw & 1]);
+        if (tw == NT - 1) { umma_commit(&dw_full[buf]); umma_commit(&w_empty[glw % C::WS]); }
+        // the same tile goes to HBM as dY (rows past the batch are clipped by the tensor map).  elect.sync names the same
+        // thread every time, so the bulk groups are this thread's: all but the newest store have been read -> the tile
+        // before this one may be overwritten as far as its store is concerned (second arrival on its s_empty)
+        tma_store_3d(&tmY, smem + C::OFF_ST + (Tw & 1) * C::ST_BYTES, 0, tw * 128, (int)(stripe + (int64_t)glw * S));
+        bulk_commit();
+        if (Tw >= 1) { bulk_wait_read<1>(); mbar_arrive(&s_empty[(Tw - 1) & 1]); }
       }
-      // ---- forward of tile Tf: gathered, W_g there, an accumulator slot free
-      if (Tf < total) {
-        const int ws = glf % C::WS, hs = Tf % C::HS, slot = Tf % C::NSLOT;
-        if (!f_w) f_w = tf != 0 || ready(&w_full[ws], (glf / C::WS) & 1);
-        if (!f_h) f_h = ready(&h_full[hs], (Tf / C::HS) & 1);
-        if (!f_t) f_t = ready(&t_empty[slot], ((Tf / C::NSLOT) & 1) ^ 1);
-        if (f_w && f_h && f_t) {
-          tc_fence_after();
-          if (elect_one()) {
-            const uint64_t ad0 = fa0 + (uint64_t)((hs * C::H_BYTES) >> 4);
-            const uint64_t bd0 = fb0 + (uint64_t)((ws * C::W_BYTES) >> 4);
-            const uint32_t d = tmem_base + C::T_FWD0 + slot * G;
-#pragma unroll
-            for (int j = 0; j < K / 16; ++j)
-              umma_f16(d, ad0 + (uint64_t)((j * 2048) >> 4), bd0 + (uint64_t)(((j >> 2) * (G * 128) + (j & 3) * 32) >> 4), idesc_f,
-                       j > 0 ? 1u : 0u);
-            umma_commit(&t_full[slot]);
-          }
-          __syncwarp();
-          f_w = f_h = f_t = false;
-          ++Tf;
-          if (++tf == NT) { tf = 0; ++glf; }
-          continue;
-        }
-      }
-      __nanosleep(32);
+      __syncwarp();
+      if (++tw == NT) { tw = 0; ++glw; }
     }
     if (elect_one()) bulk_wait<0>();
     __syncwarp();
@@ -270,7 +261,7 @@ tc_fused_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__
           tma_load_2d(smem + C::OFF_W + ws * C::W_BYTES + kb * (G * 128), &tmW, &w_full[ws], kb * 64, (int)(g * G));
       }
     }
-  } else {
+  } else if (warp < 16) {
     // ===================== epilogue: warp = (tile parity, 32-label half, TMEM lane quadrant); lane = batch row ===========
     const int q = warp & 3, half = (warp >> 2) & 1, tsel = warp >> 3;
     const int row = q * 32 + lane;
