@@ -46,6 +46,8 @@ def _alg_bytes(cfg, dw_bytes=None):
         "forward": W + idx + X + dY,
         "dW": dY + idx + X + cfg.L_t * cfg.K * dw_bytes + cfg.L_t * 4,
         "dX": dY + W + idx + dX,
+        # forward + dW in one kernel (haste_forward_loss_dw): dY is written and never read back, X is gathered once
+        "forward_dW": W + idx + X + dY + cfg.L_t * cfg.K * dw_bytes + cfg.L_t * 4,
     }
 
 
@@ -313,6 +315,7 @@ def main():
     ap.add_argument("--workload", default=WORKLOAD, help="synth.CONFIGS key (default: the 670K-label config the metric is quoted on)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-head", action="store_true", help="time the sparse tail alone")
+    ap.add_argument("--two-kernels", action="store_true", help="time the step through haste_forward_loss + haste_backward even where the one-kernel forward + dW exists")
     ap.add_argument("--deterministic", action="store_true", help="create the handles with HASTE_DETERMINISTIC (atomic-free dX)")
     ap.add_argument("--sweep", action="store_true", help="config 5: kernel sweep over B and G at K=64 against the dense bottleneck (one JSON line per point)")
     ap.add_argument("--sweep-B", default="64,256,1024")
@@ -391,12 +394,22 @@ def main():
     batches = [Batch(True), Batch(False)]
     s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
 
-    def step(b=batches[0]):
+    # forward + loss + dY + dW + db in ONE kernel where the library has it (bf16, G = 64, B <= 512: tc_fused.cu), then
+    # haste_backward for dX only; otherwise haste_forward_loss and haste_backward with all three outputs.  The same results.
+    fused_ok = layer.kernel_family == 1 and G == 64 and B <= 512 and not args.two_kernels
+
+    def step(b=batches[0], fused=None):
         n = 0
-        layer.forward_loss(B, b.X, idx, W, None, b.rowptr, b.col, loss=b.loss[0:1], dY=dY)
-        n += layer.last_launch_count
-        layer.backward(B, b.X, idx, W, dY, dW=dW, dbias=db, dX=b.dX)
-        n += layer.last_launch_count
+        if fused_ok if fused is None else fused:
+            layer.forward_loss_dw(B, b.X, idx, W, None, b.rowptr, b.col, loss=b.loss[0:1], dY=dY, dW=dW, dbias=db)
+            n += layer.last_launch_count
+            layer.backward(B, b.X, idx, W, dY, dX=b.dX)
+            n += layer.last_launch_count
+        else:
+            layer.forward_loss(B, b.X, idx, W, None, b.rowptr, b.col, loss=b.loss[0:1], dY=dY)
+            n += layer.last_launch_count
+            layer.backward(B, b.X, idx, W, dY, dW=dW, dbias=db, dX=b.dX)
+            n += layer.last_launch_count
         if use_head:
             head.forward_loss(B, b.Xh, Wh, None, b.rowptr, b.col, loss=b.loss[1:2], dY=dYh)
             n += head.last_launch_count
@@ -482,8 +495,12 @@ def main():
     if use_head:
         head.set_profiling(nprof)
     ms_prof = timed(step, args.steps)
-    kn = {"forward": haste.KERNEL_FORWARD, "dW": haste.KERNEL_DW, "dX": haste.KERNEL_DX,
-          "prep_fwd": haste.KERNEL_PREP_FWD, "prep_bwd": haste.KERNEL_PREP_BWD, "post_bwd": haste.KERNEL_POST_BWD}
+    tail_keys = ("forward_dW", "dX") if fused_ok else ("forward", "dW", "dX")
+    kn = {"dX": haste.KERNEL_DX, "prep_fwd": haste.KERNEL_PREP_FWD, "prep_bwd": haste.KERNEL_PREP_BWD, "post_bwd": haste.KERNEL_POST_BWD}
+    if fused_ok:
+        kn["forward_dW"] = haste.KERNEL_FORWARD          # the one kernel is recorded in the forward slot
+    else:
+        kn["forward"], kn["dW"] = haste.KERNEL_FORWARD, haste.KERNEL_DW
     kms = {k: [layer.kernel_ms(v, a) for a in range(nprof)] for k, v in kn.items()}
     if use_head:
         kms["head_forward"] = [head.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nprof)]
@@ -567,6 +584,22 @@ def main():
                                           "note": "one kernel for forward + loss + dY + dW + db where it exists (G = 64, B <= 512), else the two kernels; dY written once, never read back"}
         except haste.HasteError as e:
             extras["forward_dw_fused"] = {"unsupported": str(e)}
+        # ... and the two kernels that call stands for, timed the same way (haste_forward_loss, haste_backward for dW and db)
+        for _ in range(2):
+            layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY)
+            layer.backward(B, X, idx, W, dY, dW=dW, dbias=db)
+        torch.cuda.synchronize()
+        for _ in range(nx):
+            layer.forward_loss(B, X, idx, W, None, rowptr, col, loss=loss[0:1], dY=dY)
+            layer.backward(B, X, idx, W, dY, dW=dW, dbias=db)
+        torch.cuda.synchronize()
+        tf_ = [layer.kernel_ms(haste.KERNEL_FORWARD, a) for a in range(nx)]
+        tw_ = [layer.kernel_ms(haste.KERNEL_DW, a) for a in range(nx)]
+        ab2 = _alg_bytes(cfg, dw_bytes=dW.element_size())
+        extras["forward_then_dW"] = {"forward_ms": float(np.mean(tf_)), "dW_ms": float(np.mean(tw_)), "ms": float(np.mean(tf_) + np.mean(tw_)),
+                                     "forward_frac_hbm": ab2["forward"] / (float(np.mean(tf_)) * 1e-3) / 1e9 / _peaks()["hbm"],
+                                     "dW_frac_hbm": ab2["dW"] / (float(np.mean(tw_)) * 1e-3) / 1e9 / _peaks()["hbm"],
+                                     "note": "the forward kernel and the dW kernel on their own, alternating"}
     layer.set_profiling(0)
     if use_head:
         head.set_profiling(0)
@@ -590,26 +623,21 @@ def main():
         c2 = s2.stop() if rank == 0 else None
         sustained = {"steps": 200, "ms_per_step": ms_sus / 200, "clocks": c2,
                      "note": "200 more steps timed the same way after everything else; not the region `value` is computed from"}
-    # ---- the same step with forward + dW in ONE kernel (haste_forward_loss_dw, then haste_backward for dX only): the same
-    # outputs, 0.7 GB less HBM traffic per step.  At full clock it takes what the two kernels take; under the board's power
-    # management (the sustained region) it is faster.  Reported beside `value`, which stays on the two-kernel step.
-    fused_step = None
-    if 20 <= args.steps < 200 and layer.kernel_family == 1 and G == 64 and B <= 512:
-        def step_f(b=batches[0]):
-            layer.forward_loss_dw(B, b.X, idx, W, None, b.rowptr, b.col, loss=b.loss[0:1], dY=dY, dW=dW, dbias=db)
-            layer.backward(B, b.X, idx, W, dY, dX=b.dX)
-            if use_head:
-                head.forward_loss(B, b.Xh, Wh, None, b.rowptr, b.col, loss=b.loss[1:2], dY=dYh)
-                head.backward(B, b.Xh, Wh, dYh, dWh=dWh, dbias=dbh, dX=b.dXh)
+    # ---- the same step through the two separate kernels (haste_forward_loss, then haste_backward with dW, db and dX), where the
+    # timed step used the one-kernel route: the same outputs, 0.7 GB more HBM traffic per step.  Reported beside `value`.
+    two_kernel_step = None
+    if 20 <= args.steps < 200 and fused_ok:
+        def step_2(b=batches[0]):
+            step(b, fused=False)
         rest()
         for _ in range(3):
-            step_f()
+            step_2()
         torch.cuda.synchronize()
         time.sleep(0.3)
-        ms_f = timed(step_f, args.steps)
-        ms_fs = timed(step_f, 200)
-        fused_step = {"ms_per_step": ms_f / args.steps, "steps": args.steps, "sustained_ms_per_step": ms_fs / 200, "sustained_steps": 200,
-                      "note": "the step through haste_forward_loss_dw + haste_backward(dX); timed like `value` and like `sustained`"}
+        ms_2 = timed(step_2, args.steps)
+        ms_2s = timed(step_2, 200)
+        two_kernel_step = {"ms_per_step": ms_2 / args.steps, "steps": args.steps, "sustained_ms_per_step": ms_2s / 200, "sustained_steps": 200,
+                           "note": "the step through haste_forward_loss + haste_backward(dW, db, dX); timed like `value` and like `sustained`"}
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -623,11 +651,11 @@ def main():
     ab = _alg_bytes(cfg)
     SPEC_HBM, SPEC_BF16 = 8000.0, 2250.0          # B200 nominal: HBM3e GB/s, dense bf16 TFLOP/s
     kernels = {}
-    for k in ("forward", "dW", "dX"):
+    for k in tail_keys:
         mean, med = float(np.mean(kms[k])), float(np.median(kms[k]))
         gbs = ab[k] / (mean * 1e-3) / 1e9
         kernels[k] = {"ms": mean, "ms_median": med, "ms_min": float(np.min(kms[k])), "GB/s": gbs, "frac_hbm": gbs / peaks["hbm"],
-                      "frac_hbm_spec": gbs / SPEC_HBM, "TFLOP/s": tail_f / (mean * 1e-3) / 1e12, "alg_bytes": ab[k]}
+                      "frac_hbm_spec": gbs / SPEC_HBM, "TFLOP/s": (2 if k == "forward_dW" else 1) * tail_f / (mean * 1e-3) / 1e12, "alg_bytes": ab[k]}
     for k in kms:
         if k not in kernels:
             kernels[k] = {"ms": float(np.mean(kms[k])), "ms_median": float(np.median(kms[k])), "ms_min": float(np.min(kms[k]))}
@@ -640,7 +668,7 @@ def main():
         g = logits_only["alg_bytes"] / (logits_only["ms"] * 1e-3) / 1e9
         logits_only.update({"GB/s": g, "frac_hbm": g / peaks["hbm"], "frac_hbm_spec": g / SPEC_HBM})
         kernels["forward_logits_only"] = logits_only
-    dom = max(("forward", "dW", "dX"), key=lambda k: kernels[k]["ms"])
+    dom = max(tail_keys, key=lambda k: kernels[k]["ms"])
     # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture of this round.  The record names the
     # kernel and carries the SHA-256 of the kernel source it was captured from: a stale record (source changed since) gives null.
     traffic, traffic_src = None, None
@@ -673,6 +701,8 @@ def main():
         "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": "config3_670k" if args.workload == "670k" else args.workload, "B": B, "d": d, "L_tail": L, "L_head": Lh if use_head else 0,
                    "G": G, "K": K, "replicas": world, "l2": l2_note,
+                   "step_route": ("haste_forward_loss_dw (forward + loss + dY + dW + db in one kernel) + haste_backward (dX)" if fused_ok
+                                  else "haste_forward_loss + haste_backward (dW, db, dX)") + (" + head forward + head backward" if use_head else ""),
                    "kernel_family": {"tail": layer.kernel_family, "head": head.kernel_family if use_head else None}, "deterministic": bool(args.deterministic)},
         "e2e": {"value": e2e_value, "unit": "TFLOP/s", "ms_per_step": ms_e2e / args.steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "note": "copies on their own streams, two sets of device buffers; no per-kernel events"},
@@ -686,10 +716,10 @@ def main():
     if sustained:
         sustained["value"] = whole_job_tflops(world, step_flops, sustained["ms_per_step"])
         out["sustained"] = sustained
-    if fused_step:
-        fused_step["value"] = whole_job_tflops(world, step_flops, fused_step["ms_per_step"])
-        fused_step["sustained_value"] = whole_job_tflops(world, step_flops, fused_step["sustained_ms_per_step"])
-        out["step_fused_forward_dw"] = fused_step
+    if two_kernel_step:
+        two_kernel_step["value"] = whole_job_tflops(world, step_flops, two_kernel_step["ms_per_step"])
+        two_kernel_step["sustained_value"] = whole_job_tflops(world, step_flops, two_kernel_step["sustained_ms_per_step"])
+        out["step_two_kernels"] = two_kernel_step
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(cfg)
     print(json.dumps(out))
