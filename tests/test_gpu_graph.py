@@ -60,7 +60,8 @@ def test_step_captures_into_a_cuda_graph(shape):
         assert torch.allclose(out[k], ref[k], rtol=1e-4, atol=1e-6), k
 
 
-def test_back_to_back_steps_are_reproducible():
+@pytest.mark.parametrize("route", ["two_kernels", "one_kernel"])
+def test_back_to_back_steps_are_reproducible(route):
     """The step's kernels are launched with programmatic stream serialization (common.cuh): each starts while the one
     before is still draining and must not touch global memory before its griddepcontrol.wait.  A kernel that did would
     read a half-written dY, X^T or dX^T now and then.  40 steps back to back with inputs that change from step to step
@@ -86,8 +87,12 @@ def test_back_to_back_steps_are_reproducible():
                     dXh=torch.empty(B, d, device=dev()))
 
     def step(X, o):
-        layer.forward_loss(B, X, idx, W, bias, rowptr, col, loss=o["loss"][0:1], dY=o["dY"])
-        layer.backward(B, X, idx, W, o["dY"], dW=o["dW"], dbias=o["db"], dX=o["dX"])
+        if route == "one_kernel":       # forward + dW in one kernel (tc_fused.cu), then dX: the route bench.py's step takes
+            layer.forward_loss_dw(B, X, idx, W, bias, rowptr, col, loss=o["loss"][0:1], dY=o["dY"], dW=o["dW"], dbias=o["db"])
+            layer.backward(B, X, idx, W, o["dY"], dX=o["dX"])
+        else:
+            layer.forward_loss(B, X, idx, W, bias, rowptr, col, loss=o["loss"][0:1], dY=o["dY"])
+            layer.backward(B, X, idx, W, o["dY"], dW=o["dW"], dbias=o["db"], dX=o["dX"])
         head.forward_loss(B, X, Wh, None, rowptr, col, loss=o["loss"][1:2], dY=o["dYh"])
         head.backward(B, X, Wh, o["dYh"], dWh=o["dWh"], dbias=None, dX=o["dXh"])
 
